@@ -1,0 +1,150 @@
+/*
+ * vegas_b200.h -- C ABI of libvegas_b200.so: one Vegas iteration over a batch of events + the grid
+ * refinement it feeds, on one NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute is the data-parallel hot path of VegasFlow (Monte Carlo
+ * integration by "importance sampling techniques from Vegas" on "adaptive grids", where "every iteration
+ * informs the subsequent run"; user API PAPER.md:L72-L79: VegasFlow(n_dim, n_events,
+ * events_limit) / compile(integrand) / run_integration(n_iter)).  The paper prints no equation; the
+ * arithmetic is the reading S1-S7 / I0-I4 / R1-R17 of SURVEY.md section 8.c, restated in DESIGN.md.
+ *
+ * Conventions
+ *   - Plain C, no torch / CUDA types.  Pointers are HOST pointers unless the name starts with dev_.
+ *   - Every function returns an int status (VEGAS_OK = 0, negative = error) unless stated.  After an
+ *     error vegas_last_error() returns a static, thread-local, NUL-terminated description.
+ *   - The caller owns every buffer it passes.  `params` is copied at create.  `dev_workspace` (device
+ *     memory, >= vegas_workspace_bytes(), 256-byte aligned) and `cuda_stream` (a cudaStream_t cast to
+ *     void*, NULL = the legacy default stream) are borrowed and must outlive the context; the library
+ *     allocates no device memory itself except a few bytes of pinned host memory for results.
+ *   - A context is not thread-safe.  Calls that return results to host pointers are synchronous at
+ *     return (they synchronise the stream); they enqueue asynchronously inside (no host sync between
+ *     the launches of one iteration).
+ *   - There is no CPU fallback: every step runs in CUDA kernels; without a CUDA device vegas_create
+ *     fails with VEGAS_ECUDA.
+ */
+#ifndef VEGAS_B200_H
+#define VEGAS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vegas_ctx vegas_ctx; /* opaque; created by vegas_create, freed by vegas_destroy */
+
+enum {
+    VEGAS_OK = 0,
+    VEGAS_EINVAL = -1,       /* bad argument (range, NULL, wrong n_params) */
+    VEGAS_ECUDA = -2,        /* a CUDA runtime call failed / no device */
+    VEGAS_ENOMEM = -3,       /* workspace too small or host allocation failed */
+    VEGAS_ESTATE = -4,       /* call order: vegas_refine before any vegas_iterate */
+    VEGAS_EUNSUPPORTED = -5, /* no compiled kernel instance for (integrand_id, dim, nbins, precision) */
+    VEGAS_EGRID = -6         /* grid not strictly increasing from 0 to 1; grid left unchanged */
+};
+
+/* Per-event arithmetic precision (uniform, map, Jacobian, integrand).  wf, (wf)^2, all sums, the
+ * histogram, the refinement and the master edges are always fp64 (BASELINE.json configs[3]: "FP32
+ * integrand with FP64 accumulation"; reading R14). */
+enum { VEGAS_FP64 = 0, VEGAS_FP32_EVAL = 1 };
+
+/* Built-in integrands (device functions chosen at compile time; BASELINE.json north_star "Integrand
+ * evaluation") and their `params` (doubles):
+ *   0 gauss_sym      {alpha, mu}                         f = prod_k exp(-(x_k-mu)^2/alpha^2)/(alpha sqrt(pi))   configs[0]
+ *   1 gauss_double   {alpha, mu1, mu2}                   f = 1/2 [prod N(x_k;mu1,alpha) + prod N(x_k;mu2,alpha)]  configs[1],[2]
+ *   2 genz_osc_peak  {phase_fraction, c_0 .. c_{dim-1}}  f = cos(2 pi phase + sum c_k x_k) prod 1/(c_k^-2+(x_k-1/2)^2), fp32   configs[3]
+ *   3 lo_2to2        {sqrt_s, sqrt_shat_min, cos_cut, pdf_a, pdf_b=5}   synthetic LO 2->2, dim = 3          configs[4]
+ *   4 toy_sum        {}                                  f = sum_k x_k
+ */
+enum { VEGAS_GAUSS_SYM = 0, VEGAS_GAUSS_DOUBLE = 1, VEGAS_GENZ_OSC_PEAK = 2, VEGAS_LO_2TO2 = 3, VEGAS_TOY_SUM = 4 };
+
+/* Device bytes the caller must provide to vegas_create for this (dim, nbins).  0 if out of range. */
+size_t vegas_workspace_bytes(int dim, int nbins);
+
+/* Create an integrator state: uniform grid (E[k][i] = i/nbins), iteration counter 0.
+ * Mirrors VegasFlow(n_dim, ...) + compile(integrand): the integrand is selected
+ * among the compiled instances instead of being traced.
+ *   dim 1..32; nbins 2..4095 (fp64) / 2..511 (fp32) so that m*nbins is exact (S2).
+ * Errors: VEGAS_EINVAL (ranges, NULL out, n_params mismatch, misaligned workspace), VEGAS_ENOMEM
+ * (workspace_bytes too small), VEGAS_EUNSUPPORTED (no instance), VEGAS_ECUDA. */
+int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
+                 int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* One Vegas iteration (S1-S6): n_events events, global event index e in [0, n_events), cut into
+ * ceil(n_events/events_per_launch) kernel launches (PAPER.md:L57-L65 `events_limit`; results do not
+ * depend on it, reading R16).  Event e draws its point from Philox4x32-10 keyed by `seed` with counter
+ * (e, iteration, coordinate block), maps it through the grid, evaluates the integrand, and the kernels
+ * accumulate S1 = sum wf, S2 = sum (wf)^2 and H[k][bin_k] += (wf)^2.
+ *   integral = S1/n, error = sqrt(max(0,(S2/n - I^2)/(n-1))); hist (may be NULL) receives dim*nbins
+ *   doubles, row-major [k][i].  The histogram also stays on the device for vegas_refine.
+ * On success the iteration counter increments by one.  Non-finite results are returned as they are.
+ * Errors: VEGAS_EINVAL (n_events < 2, events_per_launch == 0, NULL integral/error), VEGAS_ECUDA. */
+int vegas_iterate(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
+                  double* integral, double* error, double* hist);
+
+/* Grid refinement (S7) from the histogram of the last vegas_iterate: 3-point smoothing, damping
+ * ((1-r)/ln(1/r))^alpha, rebinning to equal damped weight; rebuilds the mapping table; clears H.
+ * Errors: VEGAS_EINVAL (alpha < 0 or NaN), VEGAS_ESTATE (no histogram), VEGAS_EGRID (new edges not
+ * strictly increasing: grid unchanged), VEGAS_ECUDA. */
+int vegas_refine(vegas_ctx* ctx, double alpha);
+
+/* Master edges, fp64, dim*(nbins+1) doubles row-major [k][i].  set validates 0 = E0 < E1 < ... < EN = 1
+ * (else VEGAS_EGRID, grid unchanged) and rebuilds the table with wd = E[i+1]-E[i] (S2). */
+int vegas_get_grid(const vegas_ctx* ctx, double* edges);
+int vegas_set_grid(vegas_ctx* ctx, const double* edges);
+
+/* Uniform grid, iteration counter 0, histogram cleared. */
+int vegas_reset(vegas_ctx* ctx);
+
+/* The counter word fed to Philox as "iteration" (test hook; S1). */
+int vegas_set_iteration(vegas_ctx* ctx, uint32_t iteration);
+int vegas_get_iteration(const vegas_ctx* ctx, uint32_t* iteration);
+
+/* Parity hook: S1-S4 for events first_event .. first_event+count-1 of the current iteration counter,
+ * computed by the same device functions as vegas_iterate.  Any output pointer may be NULL.
+ *   bins [count*dim] int32, x [count*dim] (fp32 values widened to double in fp32 mode), jac [count],
+ *   f [count], wf [count] (= (double)J*(double)f), pass [count] (1 unless the integrand's cut rejected
+ *   the event). */
+int vegas_debug_events(vegas_ctx* ctx, uint64_t first_event, uint32_t count, uint64_t seed, int32_t* bins,
+                       double* x, double* jac, double* f, double* wf, int32_t* pass);
+
+/* S1, S2 of the last vegas_iterate and the device time of everything it enqueued (CUDA events on the
+ * context's stream: all launches + finalize, excluding the result copy).  Any pointer may be NULL.
+ * VEGAS_ESTATE before the first iterate. */
+int vegas_last_sums(const vegas_ctx* ctx, double* S1, double* S2, double* kernel_ms);
+
+/* Asynchronous form used for timing (bench.py): enqueue one iteration without reading results back
+ * and without synchronising; results stay on the device until vegas_iterate_collect (same outputs as
+ * vegas_iterate) which synchronises.  n_kernel_launches (may be NULL) receives how many kernels the
+ * call enqueued. */
+int vegas_iterate_enqueue(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
+                          int* n_kernel_launches);
+int vegas_iterate_collect(vegas_ctx* ctx, double* integral, double* error, double* hist);
+
+/* Launch-shape tuning knobs of the iterate kernel (the batch-size / occupancy study):
+ * CTAs per SM and threads per CTA (0 = library default 2 x 512; threads a multiple of 32, <= 1024), and
+ * the number R of lane-indexed shared-memory histogram replicas (power of two 1..32; 0 = the largest
+ * that fits).  Results do not depend on them beyond summation order.  VEGAS_EINVAL if the shape cannot
+ * run (shared memory); ctas_per_sm is clamped to what the device can hold. */
+int vegas_set_launch_shape(vegas_ctx* ctx, int ctas_per_sm, int threads_per_cta);
+int vegas_set_hist_replicas(vegas_ctx* ctx, int replicas);
+int vegas_get_launch_shape(const vegas_ctx* ctx, int* ctas_per_sm, int* threads_per_cta, int* hist_replicas,
+                           size_t* smem_bytes);
+
+/* Number of events of the last iteration whose integrand was not cut away (lo_2to2's cuts; equals
+ * n_events for the other integrands).  VEGAS_ESTATE before the first iterate. */
+int vegas_last_npass(const vegas_ctx* ctx, uint64_t* npass);
+
+void vegas_destroy(vegas_ctx* ctx);
+
+const char* vegas_last_error(void);
+
+/* Library / device facts for reports: writes the SM count and the SM clock (kHz) of the device the
+ * context runs on. */
+int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VEGAS_B200_H */

@@ -1,0 +1,612 @@
+// vegas_api.cu -- C ABI of libvegas_b200.so (include/vegas_b200.h): host driver of the Vegas hot path.
+//
+// The host side only validates arguments, lays out the caller's device workspace, cuts an iteration
+// into launches (a8, PAPER.md:L57-L65 `events_limit`) and enqueues kernels on the caller's stream.
+// Every step S1-S7 runs in the kernels of vegas_kernels.cuh; there is no CPU fallback.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <type_traits>
+
+#include <cuda_runtime.h>
+
+#include "../../include/vegas_b200.h"
+#include "vegas_kernels.cuh"
+
+namespace {
+
+using namespace vegas;
+
+constexpr int kMaxSlots = 4096;          // upper bound on the iterate grid (CTAs)
+constexpr double kPi = 0x1.921fb54442d18p+1;   // fl64(pi)
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                               \
+    do {                                                                                             \
+        cudaError_t e_ = (expr);                                                                     \
+        if (e_ != cudaSuccess)                                                                       \
+            return fail(VEGAS_ECUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---- device workspace layout (all offsets 256-byte aligned) -------------------------------------
+struct Layout {
+    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, total;
+};
+
+Layout make_layout(int dim, int nbins)
+{
+    Layout L{};
+    const size_t cells = static_cast<size_t>(dim) * nbins, nedges = static_cast<size_t>(dim) * (nbins + 1);
+    size_t o = 0;
+    L.edges = o;      o = align_up(o + nedges * 8, 256);
+    L.new_edges = o;  o = align_up(o + nedges * 8, 256);
+    L.table = o;      o = align_up(o + cells * 16, 256);
+    L.zero_begin = o;                                   // [hist | slots | npass] is cleared by one memset
+    L.hist = o;       o = align_up(o + cells * 8, 256);
+    L.slots = o;      o = align_up(o + static_cast<size_t>(kMaxSlots) * 32, 256);
+    L.npass = o;      o = align_up(o + 8, 256);
+    L.zero_end = o;
+    L.result = o;     o = align_up(o + 64, 256);
+    L.flags = o;      o = align_up(o + kMaxDim * 4, 256);
+    L.status = o;     o = align_up(o + 4, 256);
+    L.total = o;
+    return L;
+}
+
+// ---- compiled kernel instances -------------------------------------------------------------------
+using LaunchFn = cudaError_t (*)(const IterArgs&, int grid, int threads, size_t smem, cudaStream_t);
+using DebugFn = cudaError_t (*)(const IterArgs&, int grid, int threads, cudaStream_t, int32_t*, double*, double*,
+                                double*, double*, int32_t*);
+using AttrFn = cudaError_t (*)(int smem_bytes);
+using OccFn = cudaError_t (*)(int* ctas, int threads, size_t smem);
+
+struct Instance {
+    int integrand_id, dim /* 0 = any */, precision, max_threads;
+    LaunchFn launch;
+    DebugFn debug;
+    AttrFn set_smem;
+    OccFn occupancy;
+};
+
+template <class F, int D, int MAXT, int MINB>
+cudaError_t launch_iterate(const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    iterate_kernel<F, D, MAXT, MINB><<<grid, threads, smem, st>>>(a);
+    return cudaGetLastError();
+}
+template <class F, int D>
+cudaError_t launch_debug(const IterArgs& a, int grid, int threads, cudaStream_t st, int32_t* bins, double* x,
+                         double* jac, double* f, double* wf, int32_t* pass)
+{
+    debug_events_kernel<F, D><<<grid, threads, 0, st>>>(a, bins, x, jac, f, wf, pass);
+    return cudaGetLastError();
+}
+template <class F, int D, int MAXT, int MINB>
+cudaError_t set_smem_attr(int smem_bytes)
+{
+    return cudaFuncSetAttribute(iterate_kernel<F, D, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                smem_bytes);
+}
+template <class F, int D, int MAXT, int MINB>
+cudaError_t query_occupancy(int* ctas, int threads, size_t smem)
+{
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, iterate_kernel<F, D, MAXT, MINB>, threads, smem);
+}
+
+#define VEGAS_INSTANCE(ID, F, D, PREC, MAXT, MINB)                                                       \
+    Instance { ID, D, PREC, MAXT, launch_iterate<F, D, MAXT, MINB>, launch_debug<F, D>,                  \
+               set_smem_attr<F, D, MAXT, MINB>, query_occupancy<F, D, MAXT, MINB> }
+
+// Exact-dimension instances for the five configurations and the paper's toy example come first; the
+// D = 0 instances take any dimension up to kMaxDim (run-time loop bounds).
+const Instance kInstances[] = {
+    VEGAS_INSTANCE(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64, 1024, 1),          // configs[0]
+    VEGAS_INSTANCE(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64, 1024, 1),    // configs[1], [2]
+    VEGAS_INSTANCE(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL, 1024, 1),   // configs[3]
+    VEGAS_INSTANCE(VEGAS_LO_2TO2, Lo2to2, 3, VEGAS_FP64, 1024, 1),              // configs[4]
+    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<double>, 10, VEGAS_FP64, 1024, 1),
+    VEGAS_INSTANCE(VEGAS_GAUSS_SYM, GaussSym, 0, VEGAS_FP64, 1024, 1),
+    VEGAS_INSTANCE(VEGAS_GAUSS_DOUBLE, GaussDouble, 0, VEGAS_FP64, 1024, 1),
+    VEGAS_INSTANCE(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 0, VEGAS_FP32_EVAL, 1024, 1),
+    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<double>, 0, VEGAS_FP64, 1024, 1),
+    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<float>, 0, VEGAS_FP32_EVAL, 1024, 1),
+};
+
+const Instance* find_instance(int id, int dim, int precision)
+{
+    for (const Instance& in : kInstances)
+        if (in.integrand_id == id && in.precision == precision && in.dim == dim) return &in;
+    for (const Instance& in : kInstances)
+        if (in.integrand_id == id && in.precision == precision && in.dim == 0) return &in;
+    return nullptr;
+}
+
+int expected_params(int id, int dim)
+{
+    switch (id) {
+        case VEGAS_GAUSS_SYM: return 2;
+        case VEGAS_GAUSS_DOUBLE: return 3;
+        case VEGAS_GENZ_OSC_PEAK: return 1 + dim;
+        case VEGAS_LO_2TO2: return 5;
+        case VEGAS_TOY_SUM: return 0;
+        default: return -1;
+    }
+}
+
+}  // namespace
+
+struct vegas_ctx {
+    int dim, nbins, integrand_id, precision;
+    const Instance* inst;
+    cudaStream_t stream;
+    unsigned char* ws;
+    Layout L;
+    IntegrandConsts ic;
+    uint32_t iteration;
+    bool have_hist, have_sums;
+    int sm_count, sm_clock_khz, smem_optin;
+    int ctas_per_sm, threads, rshift;            // launch shape in use
+    size_t smem_bytes;
+    double* h_result;        // pinned: result[8] then hist[dim*nbins]
+    int* h_status;           // pinned
+    cudaEvent_t ev0, ev1;
+    uint64_t last_n;
+    int last_launches;
+};
+
+namespace {
+
+// Integrand constants (I0-I3), one correctly rounded host operation per step (compiled with
+// -ffp-contract=off): the same statement of the constants as DESIGN.md, independent of oracle/.
+int setup_integrand(vegas_ctx* c, const double* p)
+{
+    std::memset(&c->ic, 0, sizeof(c->ic));
+    switch (c->integrand_id) {
+        case VEGAS_GAUSS_SYM:
+        case VEGAS_GAUSS_DOUBLE: {
+            const double alpha = p[0];
+            const double b = alpha * std::sqrt(kPi);
+            double C = 1.0;
+            for (int k = 0; k < c->dim; ++k) C = C / b;
+            c->ic.gC = C;
+            c->ic.ga2 = 1.0 / (alpha * alpha);
+            c->ic.gmu0 = p[1];
+            c->ic.gmu1 = (c->integrand_id == VEGAS_GAUSS_DOUBLE) ? p[2] : 0.0;
+            return VEGAS_OK;
+        }
+        case VEGAS_GENZ_OSC_PEAK: {
+            c->ic.zphi = static_cast<float>((2.0 * kPi) * p[0]);
+            for (int k = 0; k < c->dim; ++k) {
+                const float ck = static_cast<float>(p[1 + k]);
+                c->ic.zc[k] = ck;
+                c->ic.zw[k] = 1.0f / (ck * ck);
+            }
+            return VEGAS_OK;
+        }
+        case VEGAS_LO_2TO2: {
+            if (c->dim != 3) return fail(VEGAS_EINVAL, "lo_2to2 needs dim = 3");
+            if (p[4] != 5.0) return fail(VEGAS_EUNSUPPORTED, "lo_2to2: pdf_b is fixed to 5");
+            const double s = p[0] * p[0];
+            const double smin = p[1] * p[1];
+            const double tau = smin / s;
+            c->ic.hs = s;
+            c->ic.hL = std::log(tau);
+            c->ic.hcut = p[2];
+            c->ic.ha = p[3];
+            return VEGAS_OK;
+        }
+        default: return VEGAS_OK;
+    }
+}
+
+size_t iterate_smem_bytes(const vegas_ctx* c, int rshift, int threads)
+{
+    const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
+    const size_t cell_bytes = (c->precision == VEGAS_FP64) ? 16 : 8;
+    return cells * (size_t(1) << rshift) * 8 + align_up(cells * cell_bytes, 16) + static_cast<size_t>((threads + 31) / 32) * 5 * 8;
+}
+
+// Choose R = 2^rshift: the largest power of two <= 32 such that `ctas` CTAs fit in the SM's shared memory.
+int pick_rshift(const vegas_ctx* c, int ctas, int threads)
+{
+    const size_t per_sm = 228u * 1024u;
+    for (int rs = 5; rs >= 0; --rs) {
+        const size_t need = iterate_smem_bytes(c, rs, threads) + 1024;   // 1 KB reserved per CTA
+        if (need * ctas <= per_sm && need - 1024 <= static_cast<size_t>(c->smem_optin)) return rs;
+    }
+    return -1;
+}
+
+int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
+{
+    if (threads < 32 || threads > c->inst->max_threads || (threads & 31)) return fail(VEGAS_EINVAL, "threads_per_cta %d not in 32..%d (multiple of 32)", threads, c->inst->max_threads);
+    if (ctas < 1 || ctas > 16) return fail(VEGAS_EINVAL, "ctas_per_sm %d not in 1..16", ctas);
+    if (rshift < 0) rshift = pick_rshift(c, ctas, threads);
+    if (rshift < 0 || rshift > 5) return fail(VEGAS_EINVAL, "histogram of %d x %d cells does not fit in shared memory with %d CTAs/SM", c->dim, c->nbins, ctas);
+    const size_t smem = iterate_smem_bytes(c, rshift, threads);
+    if (smem > static_cast<size_t>(c->smem_optin)) return fail(VEGAS_EINVAL, "needs %zu bytes of shared memory per CTA, device allows %d", smem, c->smem_optin);
+    CUDA_TRY(c->inst->set_smem(static_cast<int>(smem)));
+    int occ = 0;
+    CUDA_TRY(c->inst->occupancy(&occ, threads, smem));
+    if (occ < 1) return fail(VEGAS_EINVAL, "launch shape (%d threads, %zu B smem) cannot run", threads, smem);
+    if (occ < ctas) ctas = occ;
+    if (ctas * c->sm_count > kMaxSlots) ctas = kMaxSlots / c->sm_count;
+    c->ctas_per_sm = ctas; c->threads = threads; c->rshift = rshift; c->smem_bytes = smem;
+    return VEGAS_OK;
+}
+
+void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count, IterArgs& a)
+{
+    a.table = c->ws + c->L.table;
+    a.hist = reinterpret_cast<double*>(c->ws + c->L.hist);
+    a.slots = reinterpret_cast<double*>(c->ws + c->L.slots);
+    a.npass = reinterpret_cast<unsigned long long*>(c->ws + c->L.npass);
+    a.e_lo_first = static_cast<uint32_t>(first);
+    a.e_hi = static_cast<uint32_t>(first >> 32);
+    a.count = count;
+    a.iteration = c->iteration;
+    const uint32_t k0 = static_cast<uint32_t>(seed), k1 = static_cast<uint32_t>(seed >> 32);
+    for (int r = 0; r < 10; ++r) {
+        a.rk0[r] = k0 + static_cast<uint32_t>(r) * 0x9E3779B9u;
+        a.rk1[r] = k1 + static_cast<uint32_t>(r) * 0xBB67AE85u;
+    }
+    a.dim = c->dim;
+    a.nbins = c->nbins;
+    a.rshift = c->rshift;
+    a.ic = c->ic;
+}
+
+int build_table(vegas_ctx* c, int uniform)
+{
+    build_table_kernel<<<c->dim, 128, 0, c->stream>>>(reinterpret_cast<double*>(c->ws + c->L.edges),
+                                                      c->ws + c->L.table, c->nbins, c->precision, uniform);
+    CUDA_TRY(cudaGetLastError());
+    return VEGAS_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// extern "C" entry points (documented in include/vegas_b200.h)
+// =================================================================================================
+extern "C" {
+
+const char* vegas_last_error(void) { return g_err; }
+
+size_t vegas_workspace_bytes(int dim, int nbins)
+{
+    if (dim < 1 || dim > kMaxDim || nbins < 2 || nbins > 4095) return 0;
+    return make_layout(dim, nbins).total;
+}
+
+int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
+                 int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out) return fail(VEGAS_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (dim < 1 || dim > kMaxDim) return fail(VEGAS_EINVAL, "dim %d not in 1..%d", dim, kMaxDim);
+    if (precision != VEGAS_FP64 && precision != VEGAS_FP32_EVAL) return fail(VEGAS_EINVAL, "precision %d unknown", precision);
+    const int max_bins = (precision == VEGAS_FP64) ? 4095 : 511;     // m*N must be exact (S2)
+    if (nbins < 2 || nbins > max_bins) return fail(VEGAS_EINVAL, "nbins %d not in 2..%d", nbins, max_bins);
+    const int need = expected_params(integrand_id, dim);
+    if (need < 0) return fail(VEGAS_EUNSUPPORTED, "integrand_id %d unknown", integrand_id);
+    if (n_params != need || (need > 0 && !params)) return fail(VEGAS_EINVAL, "integrand %d with dim %d takes %d params, got %d", integrand_id, dim, need, n_params);
+    const Instance* inst = find_instance(integrand_id, dim, precision);
+    if (!inst) return fail(VEGAS_EUNSUPPORTED, "no compiled kernel for integrand %d, dim %d, precision %d", integrand_id, dim, precision);
+    if (!dev_workspace) return fail(VEGAS_EINVAL, "dev_workspace is NULL");
+    if (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) return fail(VEGAS_EINVAL, "dev_workspace must be 256-byte aligned");
+    const Layout L = make_layout(dim, nbins);
+    if (workspace_bytes < L.total) return fail(VEGAS_ENOMEM, "workspace of %zu bytes, need %zu", workspace_bytes, L.total);
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        (void)cudaGetLastError();
+        return fail(VEGAS_ECUDA, "no CUDA device (there is no CPU fallback)");
+    }
+    vegas_ctx* c = new (std::nothrow) vegas_ctx();
+    if (!c) return fail(VEGAS_ENOMEM, "host allocation failed");
+    c->dim = dim; c->nbins = nbins; c->integrand_id = integrand_id; c->precision = precision;
+    c->inst = inst;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->ws = static_cast<unsigned char*>(dev_workspace);
+    c->L = L;
+    c->iteration = 0; c->have_hist = false; c->have_sums = false;
+    c->h_result = nullptr; c->h_status = nullptr; c->ev0 = nullptr; c->ev1 = nullptr;
+    c->last_n = 0; c->last_launches = 0;
+    int rc = setup_integrand(c, params);
+    if (rc != VEGAS_OK) { delete c; return rc; }
+
+    auto cleanup = [&](int code) { vegas_destroy(c); return code; };
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
+        return cleanup(fail(VEGAS_ECUDA, "cudaGetDeviceProperties failed"));
+    if (prop.major < 10) return cleanup(fail(VEGAS_ECUDA, "device sm_%d%d: this library is built for sm_100a only", prop.major, prop.minor));
+    c->sm_count = prop.multiProcessorCount;
+    c->smem_optin = static_cast<int>(prop.sharedMemPerBlockOptin);
+    int khz = 0;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+    c->sm_clock_khz = khz;
+    if (cudaHostAlloc(reinterpret_cast<void**>(&c->h_result), (8 + static_cast<size_t>(dim) * nbins) * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
+        cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess)
+        return cleanup(fail(VEGAS_ECUDA, "pinned host buffer / event creation failed: %s", cudaGetErrorString(cudaGetLastError())));
+    rc = apply_shape(c, 2, 512, -1);
+    if (rc != VEGAS_OK) rc = apply_shape(c, 1, 512, -1);
+    if (rc != VEGAS_OK) return cleanup(rc);
+    if (cudaMemsetAsync(c->ws, 0, L.total, c->stream) != cudaSuccess) return cleanup(fail(VEGAS_ECUDA, "workspace memset failed"));
+    rc = build_table(c, 1);
+    if (rc != VEGAS_OK) return cleanup(rc);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return cleanup(fail(VEGAS_ECUDA, "create: %s", cudaGetErrorString(cudaGetLastError())));
+    *out = c;
+    return VEGAS_OK;
+}
+
+void vegas_destroy(vegas_ctx* c)
+{
+    if (!c) return;
+    if (c->h_result) cudaFreeHost(c->h_result);
+    if (c->h_status) cudaFreeHost(c->h_status);
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
+    delete c;
+}
+
+int vegas_set_launch_shape(vegas_ctx* c, int ctas_per_sm, int threads_per_cta)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    return apply_shape(c, ctas_per_sm > 0 ? ctas_per_sm : 2, threads_per_cta > 0 ? threads_per_cta : 512, -1);
+}
+
+int vegas_set_hist_replicas(vegas_ctx* c, int replicas)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    int rs = -1;
+    if (replicas > 0) {
+        for (rs = 0; rs <= 5 && (1 << rs) != replicas; ++rs) {}
+        if (rs > 5) return fail(VEGAS_EINVAL, "replicas must be a power of two in 1..32");
+    }
+    return apply_shape(c, c->ctas_per_sm, c->threads, rs);
+}
+
+int vegas_get_launch_shape(const vegas_ctx* c, int* ctas_per_sm, int* threads_per_cta, int* hist_replicas,
+                           size_t* smem_bytes)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (ctas_per_sm) *ctas_per_sm = c->ctas_per_sm;
+    if (threads_per_cta) *threads_per_cta = c->threads;
+    if (hist_replicas) *hist_replicas = 1 << c->rshift;
+    if (smem_bytes) *smem_bytes = c->smem_bytes;
+    return VEGAS_OK;
+}
+
+int vegas_device_info(const vegas_ctx* c, int* sm_count, int* sm_clock_khz)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (sm_count) *sm_count = c->sm_count;
+    if (sm_clock_khz) *sm_clock_khz = c->sm_clock_khz;
+    return VEGAS_OK;
+}
+
+int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
+                          int* n_kernel_launches)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (n_events < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
+    if (events_per_launch == 0) return fail(VEGAS_EINVAL, "events_per_launch must be > 0");
+    if (n_events > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
+    const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
+    CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
+    CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    IterArgs a;
+    fill_args(c, seed, 0, 0, a);
+    const int max_grid = c->ctas_per_sm * c->sm_count;
+    int launches = 0, used_grid = 0;
+    for (uint64_t done = 0; done < n_events;) {
+        uint64_t cnt = n_events - done;
+        if (cnt > epl) cnt = epl;
+        const uint64_t to_wrap = (uint64_t(1) << 32) - (done & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
+        if (cnt > to_wrap) cnt = to_wrap;
+        a.e_lo_first = static_cast<uint32_t>(done);
+        a.e_hi = static_cast<uint32_t>(done >> 32);
+        a.count = static_cast<uint32_t>(cnt);
+        const uint64_t want = (cnt + c->threads - 1) / c->threads;
+        const int grid = want < static_cast<uint64_t>(max_grid) ? static_cast<int>(want) : max_grid;
+        CUDA_TRY(c->inst->launch(a, grid, c->threads, c->smem_bytes, c->stream));
+        if (grid > used_grid) used_grid = grid;
+        done += cnt;
+        ++launches;
+    }
+    finalize_kernel<<<1, 32, 0, c->stream>>>(reinterpret_cast<const double*>(c->ws + c->L.slots), used_grid,
+                                             reinterpret_cast<const unsigned long long*>(c->ws + c->L.npass),
+                                             n_events, reinterpret_cast<double*>(c->ws + c->L.result));
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaEventRecord(c->ev1, c->stream));
+    c->iteration += 1;
+    c->have_hist = true;
+    c->have_sums = true;
+    c->last_n = n_events;
+    c->last_launches = launches + 1;
+    if (n_kernel_launches) *n_kernel_launches = launches + 1;
+    return VEGAS_OK;
+}
+
+int vegas_iterate_collect(vegas_ctx* c, double* integral, double* error, double* hist)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!integral || !error) return fail(VEGAS_EINVAL, "integral and error are required");
+    if (!c->have_sums) return fail(VEGAS_ESTATE, "no iteration has been enqueued");
+    const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
+    CUDA_TRY(cudaMemcpyAsync(c->h_result, c->ws + c->L.result, 64, cudaMemcpyDeviceToHost, c->stream));
+    if (hist) CUDA_TRY(cudaMemcpyAsync(c->h_result + 8, c->ws + c->L.hist, cells * 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    *integral = c->h_result[0];
+    *error = c->h_result[1];
+    if (hist) std::memcpy(hist, c->h_result + 8, cells * 8);
+    return VEGAS_OK;
+}
+
+int vegas_iterate(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed, double* integral,
+                  double* error, double* hist)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!integral || !error) return fail(VEGAS_EINVAL, "integral and error are required");
+    const int rc = vegas_iterate_enqueue(c, n_events, events_per_launch, seed, nullptr);
+    if (rc != VEGAS_OK) return rc;
+    return vegas_iterate_collect(c, integral, error, hist);
+}
+
+int vegas_last_sums(const vegas_ctx* c, double* S1, double* S2, double* kernel_ms)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!c->have_sums) return fail(VEGAS_ESTATE, "no iteration yet");
+    CUDA_TRY(cudaMemcpyAsync(c->h_result, c->ws + c->L.result, 64, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (S1) *S1 = c->h_result[2];
+    if (S2) *S2 = c->h_result[3];
+    if (kernel_ms) {
+        float ms = 0.f;
+        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+        *kernel_ms = ms;
+    }
+    return VEGAS_OK;
+}
+
+int vegas_last_npass(const vegas_ctx* c, uint64_t* npass)
+{
+    if (!c || !npass) return fail(VEGAS_EINVAL, "NULL argument");
+    if (!c->have_sums) return fail(VEGAS_ESTATE, "no iteration yet");
+    CUDA_TRY(cudaMemcpyAsync(c->h_result, c->ws + c->L.result, 64, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    *npass = static_cast<uint64_t>(c->h_result[4]);
+    return VEGAS_OK;
+}
+
+int vegas_refine(vegas_ctx* c, double alpha)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
+    if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
+    const int N = c->nbins;
+    const size_t smem = (3 * static_cast<size_t>(N) + 1) * sizeof(double);
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    double* edges = reinterpret_cast<double*>(c->ws + c->L.edges);
+    double* new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);
+    double* hist = reinterpret_cast<double*>(c->ws + c->L.hist);
+    int* flags = reinterpret_cast<int*>(c->ws + c->L.flags);
+    int* status = reinterpret_cast<int*>(c->ws + c->L.status);
+    refine_kernel<<<c->dim, 128, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags);
+    CUDA_TRY(cudaGetLastError());
+    refine_commit_kernel<<<c->dim, 128, 0, c->stream>>>(edges, new_edges, flags, c->dim, N, c->ws + c->L.table,
+                                                        c->precision, hist, status);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(c->h_status, status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    if (c->h_status[0] != 0) return fail(VEGAS_EGRID, "refined edges are not strictly increasing; grid unchanged");
+    c->have_hist = false;
+    return VEGAS_OK;
+}
+
+int vegas_get_grid(const vegas_ctx* c, double* edges)
+{
+    if (!c || !edges) return fail(VEGAS_EINVAL, "NULL argument");
+    CUDA_TRY(cudaMemcpyAsync(edges, c->ws + c->L.edges, static_cast<size_t>(c->dim) * (c->nbins + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return VEGAS_OK;
+}
+
+int vegas_set_grid(vegas_ctx* c, const double* edges)
+{
+    if (!c || !edges) return fail(VEGAS_EINVAL, "NULL argument");
+    const int d = c->dim, N = c->nbins;
+    for (int k = 0; k < d; ++k) {                       // argument validation (host pointer)
+        const double* E = edges + static_cast<size_t>(k) * (N + 1);
+        if (E[0] != 0.0 || E[N] != 1.0) return fail(VEGAS_EGRID, "dimension %d: edges must run from 0 to 1", k);
+        for (int i = 0; i < N; ++i)
+            if (!(E[i] < E[i + 1])) return fail(VEGAS_EGRID, "dimension %d: edges not strictly increasing at %d", k, i);
+    }
+    CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.edges, edges, static_cast<size_t>(d) * (N + 1) * 8, cudaMemcpyHostToDevice, c->stream));
+    const int rc = build_table(c, 0);
+    if (rc != VEGAS_OK) return rc;
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    return VEGAS_OK;
+}
+
+int vegas_reset(vegas_ctx* c)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    const int rc = build_table(c, 1);
+    if (rc != VEGAS_OK) return rc;
+    CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    c->iteration = 0;
+    c->have_hist = false;
+    c->have_sums = false;
+    return VEGAS_OK;
+}
+
+int vegas_set_iteration(vegas_ctx* c, uint32_t iteration)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    c->iteration = iteration;
+    return VEGAS_OK;
+}
+
+int vegas_get_iteration(const vegas_ctx* c, uint32_t* iteration)
+{
+    if (!c || !iteration) return fail(VEGAS_EINVAL, "NULL argument");
+    *iteration = c->iteration;
+    return VEGAS_OK;
+}
+
+int vegas_debug_events(vegas_ctx* c, uint64_t first_event, uint32_t count, uint64_t seed, int32_t* bins, double* x,
+                       double* jac, double* f, double* wf, int32_t* pass)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (count == 0) return VEGAS_OK;
+    if ((first_event & 0xFFFFFFFFull) + count > (uint64_t(1) << 32)) return fail(VEGAS_EINVAL, "range straddles a multiple of 2^32");
+    const size_t d = static_cast<size_t>(c->dim);
+    const size_t b_bins = align_up(count * d * 4, 256), b_x = align_up(count * d * 8, 256), b_s = align_up(static_cast<size_t>(count) * 8, 256),
+                 b_p = align_up(static_cast<size_t>(count) * 4, 256);
+    unsigned char* tmp = nullptr;                        // temporary device buffer, freed before return
+    CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&tmp), b_bins + b_x + 3 * b_s + b_p));
+    int32_t* d_bins = reinterpret_cast<int32_t*>(tmp);
+    double* d_x = reinterpret_cast<double*>(tmp + b_bins);
+    double* d_jac = reinterpret_cast<double*>(tmp + b_bins + b_x);
+    double* d_f = reinterpret_cast<double*>(tmp + b_bins + b_x + b_s);
+    double* d_wf = reinterpret_cast<double*>(tmp + b_bins + b_x + 2 * b_s);
+    int32_t* d_pass = reinterpret_cast<int32_t*>(tmp + b_bins + b_x + 3 * b_s);
+    IterArgs a;
+    fill_args(c, seed, first_event, count, a);
+    cudaError_t e = c->inst->debug(a, static_cast<int>((count + 127) / 128), 128, c->stream, d_bins, d_x, d_jac, d_f, d_wf, d_pass);
+    auto copy = [&](void* dst, const void* src, size_t n) {
+        if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToHost, c->stream);
+    };
+    copy(bins, d_bins, count * d * 4);
+    copy(x, d_x, count * d * 8);
+    copy(jac, d_jac, static_cast<size_t>(count) * 8);
+    copy(f, d_f, static_cast<size_t>(count) * 8);
+    copy(wf, d_wf, static_cast<size_t>(count) * 8);
+    copy(pass, d_pass, static_cast<size_t>(count) * 4);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(VEGAS_ECUDA, "vegas_debug_events: %s", cudaGetErrorString(e));
+    return VEGAS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,303 @@
+// vegas_device.cuh -- per-event device functions of the Vegas hot path (sm_100a).
+//
+// Steps S1-S4 of the reading in DESIGN.md / SURVEY.md 8.c (the paper only names the method,
+// PAPER.md:L11, L21-L25, L88): S1 counter-based random stream, S2 integer-exact grid map, S3 integrand,
+// S4 weight.  Everything here stays in registers; the only memory touched is the (lo, wd) mapping table
+// in shared memory.  No code is shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace vegas {
+
+constexpr int kMaxDim = 32;
+
+// ------------------------------------------------------------------------------------------------
+// Kernel arguments (one struct, passed __grid_constant__ so that round keys and integrand constants
+// are constant-bank operands).
+// ------------------------------------------------------------------------------------------------
+struct IntegrandConsts {
+    // I0 / I1 (gauss_sym, gauss_double): C = (alpha sqrt(pi))^-d, a2 = 1/alpha^2, mu[2]
+    double gC, ga2, gmu0, gmu1;
+    // I3 (lo_2to2): s, L = log(tau), cos_cut, pdf_a
+    double hs, hL, hcut, ha;
+    // I2 (genz_osc_peak), fp32: phi, c_k, w_k = 1/c_k^2
+    float zphi;
+    float zc[kMaxDim];
+    float zw[kMaxDim];
+};
+
+struct IterArgs {
+    const void* table;     // device: (lo, wd) per cell, [dim][nbins], double2 (fp64) or float2 (fp32)
+    double* hist;          // device: H[dim][nbins], accumulated with global fp64 reductions at CTA exit
+    double* slots;         // device: per-CTA compensated accumulators [grid][4] = S1.hi, S1.lo, S2.hi, S2.lo
+    unsigned long long* npass;  // device: number of events whose integrand was not cut away
+    uint32_t e_lo_first;   // low word of the first global event index of this launch
+    uint32_t e_hi;         // high word (uniform within a launch: launches never straddle 2^32)
+    uint32_t count;        // events in this launch (<= 2^31)
+    uint32_t iteration;    // Philox counter word 2
+    uint32_t rk0[10], rk1[10];  // Philox round keys: k + r * Weyl
+    int dim, nbins;
+    int rshift;            // log2 of the number R of lane-indexed histogram replicas in shared memory
+    IntegrandConsts ic;
+};
+
+// ------------------------------------------------------------------------------------------------
+// S1 -- Philox4x32-10 (Salmon et al. 2011): multipliers 0xD2511F53 / 0xCD9E8D57, ten rounds, round
+// function (hi(M1 c2)^c1^k0, lo(M1 c2), hi(M0 c0)^c3^k1, lo(M0 c0)).  Round keys come precomputed.
+// VEGAS_PHILOX_MULHI selects hi/lo by two instructions (IMAD.HI + IMAD) instead of one IMAD.WIDE.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void mulhilo(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo)
+{
+#ifdef VEGAS_PHILOX_MULHI
+    hi = __umulhi(a, b);
+    lo = a * b;
+#else
+    const uint64_t p = static_cast<uint64_t>(a) * static_cast<uint64_t>(b);
+    hi = static_cast<uint32_t>(p >> 32);
+    lo = static_cast<uint32_t>(p);
+#endif
+}
+
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                              const IterArgs& a, uint32_t r[4])
+{
+#pragma unroll
+    for (int i = 0; i < 10; ++i) {
+        uint32_t h0, l0, h1, l1;
+        mulhilo(0xD2511F53u, c0, h0, l0);
+        mulhilo(0xCD9E8D57u, c2, h1, l1);
+        const uint32_t n0 = h1 ^ c1 ^ a.rk0[i];
+        const uint32_t n2 = h0 ^ c3 ^ a.rk1[i];
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+    }
+    r[0] = c0; r[1] = c1; r[2] = c2; r[3] = c3;
+}
+
+// ------------------------------------------------------------------------------------------------
+// S2 -- integer-exact bin rule and interpolation.
+//   fp64: m = 52-bit mantissa from words (lo, hi); p = m*N exactly; i = p>>52; frac = (p mod 2^52)/2^52.
+//         m*N = hi*(N<<20) + (lo>>12)*N   (N < 2^12, so every term fits 64 bits).
+//   fp32: m = r>>9 (23 bits); p = m*N (N < 2^9); i = p>>23; frac = (p mod 2^23)/2^23.
+// frac is built by OR-ing the remainder under the exponent of 1.0 and subtracting 1.0 (one exact add).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void bin_frac64(uint32_t w_lo, uint32_t w_hi, uint32_t N, int& i, double& frac)
+{
+    const uint64_t p = static_cast<uint64_t>(w_hi) * static_cast<uint64_t>(N << 20) +
+                       static_cast<uint64_t>(w_lo >> 12) * static_cast<uint64_t>(N);
+    const uint32_t phi = static_cast<uint32_t>(p >> 32);
+    i = static_cast<int>(phi >> 20);
+    const uint32_t fh = (phi & 0x000FFFFFu) | 0x3FF00000u;
+    frac = __dadd_rn(__hiloint2double(static_cast<int>(fh), static_cast<int>(static_cast<uint32_t>(p))), -1.0);
+}
+
+__device__ __forceinline__ void bin_frac32(uint32_t w, uint32_t N, int& i, float& frac)
+{
+    const uint32_t p = (w >> 9) * N;
+    i = static_cast<int>(p >> 23);
+    frac = __fadd_rn(__uint_as_float((p & 0x007FFFFFu) | 0x3F800000u), -1.0f);
+}
+
+// ------------------------------------------------------------------------------------------------
+// S3 -- integrands as streaming accumulators: begin(), coord(k, x_k) in ascending k, end() -> f.
+// Evaluation order is the normative one of SURVEY.md 8.c I0-I4; every fused multiply-add is explicit
+// and every other product/sum uses the non-contracting intrinsics.
+// ------------------------------------------------------------------------------------------------
+struct GaussSym {            // I0, BASELINE.json configs[0]
+    using real = double;
+    static constexpr int kId = 0;
+    double s;
+    __device__ __forceinline__ void begin(const IntegrandConsts&) { s = 0.0; }
+    __device__ __forceinline__ void coord(int, double x, const IntegrandConsts& c)
+    {
+        const double dx = __dsub_rn(x, c.gmu0);
+        s = __fma_rn(dx, dx, s);
+    }
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    {
+        pass = true;
+        return __dmul_rn(c.gC, exp(-__dmul_rn(s, c.ga2)));
+    }
+};
+
+struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
+    using real = double;
+    static constexpr int kId = 1;
+    double s1, s2;
+    __device__ __forceinline__ void begin(const IntegrandConsts&) { s1 = 0.0; s2 = 0.0; }
+    __device__ __forceinline__ void coord(int, double x, const IntegrandConsts& c)
+    {
+        const double d1 = __dsub_rn(x, c.gmu0), d2 = __dsub_rn(x, c.gmu1);
+        s1 = __fma_rn(d1, d1, s1);
+        s2 = __fma_rn(d2, d2, s2);
+    }
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    {
+        pass = true;
+        const double e1 = exp(-__dmul_rn(s1, c.ga2));
+        const double e2 = exp(-__dmul_rn(s2, c.ga2));
+        return __dmul_rn(__dmul_rn(0.5, c.gC), __dadd_rn(e1, e2));
+    }
+};
+
+// cos_f32 of I2: Cody-Waite reduction by pi/2 in three fp32 pieces + Taylor polynomials, all explicit
+// fmaf, so that the value is bit-identical to the CPU statement of the same recipe (valid |a| <= 128).
+__device__ __forceinline__ float cos_f32(float a)
+{
+    const float qf = rintf(__fmul_rn(a, 0x1.45f306p-1f));          // rnd32(2/pi)
+    float r = __fmaf_rn(qf, -0x1.921fb6p+0f, a);                    // rnd32(pi/2)
+    r = __fmaf_rn(qf, 0x1.777a5cp-25f, r);                          // -rnd32(pi/2 - C1)
+    r = __fmaf_rn(qf, 0x1.ee59dap-50f, r);                          // -rnd32(pi/2 - C1 - C2)
+    const float z = __fmul_rn(r, r);
+    float pc = -0x1.27e4fcp-22f;                                    // -1/10!
+    pc = __fmaf_rn(pc, z, 0x1.a01a02p-16f);                         //  1/8!
+    pc = __fmaf_rn(pc, z, -0x1.6c16c2p-10f);                        // -1/6!
+    pc = __fmaf_rn(pc, z, 0x1.555556p-5f);                          //  1/4!
+    pc = __fmaf_rn(pc, z, -0.5f);
+    pc = __fmaf_rn(pc, z, 1.0f);
+    float ps = -0x1.ae6456p-26f;                                    // -1/11!
+    ps = __fmaf_rn(ps, z, 0x1.71de3ap-19f);                         //  1/9!
+    ps = __fmaf_rn(ps, z, -0x1.a01a02p-13f);                        // -1/7!
+    ps = __fmaf_rn(ps, z, 0x1.111112p-7f);                          //  1/5!
+    ps = __fmaf_rn(ps, z, -0x1.555556p-3f);                         // -1/3!
+    const float sn = __fmaf_rn(__fmul_rn(z, r), ps, r);
+    const int q = static_cast<int>(qf) & 3;
+    const float v = (q & 1) ? sn : pc;
+    return (q == 1 || q == 2) ? -v : v;
+}
+
+struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event arithmetic
+    using real = float;
+    static constexpr int kId = 2;
+    float arg, Q;
+    __device__ __forceinline__ void begin(const IntegrandConsts& c) { arg = c.zphi; Q = 1.0f; }
+    __device__ __forceinline__ void coord(int k, float x, const IntegrandConsts& c)
+    {
+        arg = __fmaf_rn(c.zc[k], x, arg);
+        const float dx = __fsub_rn(x, 0.5f);
+        const float pk = __fmaf_rn(dx, dx, c.zw[k]);
+        Q = __fmul_rn(Q, pk);
+    }
+    __device__ __forceinline__ float end(const IntegrandConsts&, int, bool& pass)
+    {
+        pass = true;
+        return __fdiv_rn(cos_f32(arg), Q);
+    }
+};
+
+struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, v3)
+    using real = double;
+    static constexpr int kId = 3;
+    double v[3];
+    __device__ __forceinline__ void begin(const IntegrandConsts&) {}
+    __device__ __forceinline__ void coord(int k, double x, const IntegrandConsts&)
+    {
+        if (k == 0) v[0] = x; else if (k == 1) v[1] = x; else v[2] = x;
+    }
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    {
+        const double v1 = v[0], v2 = v[1], v3 = v[2];
+        const double L = c.hL, s = c.hs;
+        const double cth = __fma_rn(2.0, v3, -1.0);
+        pass = (__dadd_rn(v1, v2) < 1.0) && (fabs(cth) < c.hcut);   // cuts on exactly rounded quantities
+        if (!pass) return 0.0;
+        const double x1 = exp(__dmul_rn(v1, L));
+        const double x2 = exp(__dmul_rn(v2, L));
+        const double x12 = __dmul_rn(x1, x2);
+        const double shat = __dmul_rn(x12, s);
+        const double mh = __dmul_rn(-0.5, shat);
+        const double that = __dmul_rn(mh, __dsub_rn(1.0, cth));
+        const double uhat = __dmul_rn(mh, __dadd_rn(1.0, cth));
+        const double ME = __ddiv_rn(__dadd_rn(__dmul_rn(shat, shat), __dmul_rn(uhat, uhat)), __dmul_rn(that, that));
+        const double y1 = __dsub_rn(1.0, x1), y2 = __dsub_rn(1.0, x2);
+        const double y1s = __dmul_rn(y1, y1), y2s = __dmul_rn(y2, y2);
+        const double y1p5 = __dmul_rn(__dmul_rn(y1s, y1s), y1);
+        const double y2p5 = __dmul_rn(__dmul_rn(y2s, y2s), y2);
+        const double g1 = __dmul_rn(exp(__dmul_rn(-c.ha, __dmul_rn(v1, L))), y1p5);
+        const double g2 = __dmul_rn(exp(__dmul_rn(-c.ha, __dmul_rn(v2, L))), y2p5);
+        const double flux = __ddiv_rn(1.0, __dmul_rn(2.0, shat));
+        const double Jac = __dmul_rn(__dmul_rn(x12, __dmul_rn(L, L)), 2.0);
+        return __dmul_rn(__dmul_rn(__dmul_rn(__dmul_rn(g1, g2), ME), flux), Jac);
+    }
+};
+
+template <typename Real>
+struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1)
+    using real = Real;
+    static constexpr int kId = 4;
+    Real f;
+    __device__ __forceinline__ void begin(const IntegrandConsts&) { f = Real(0); }
+    __device__ __forceinline__ void coord(int, Real x, const IntegrandConsts&)
+    {
+        if constexpr (sizeof(Real) == 8) f = __dadd_rn(f, x); else f = __fadd_rn(f, x);
+    }
+    __device__ __forceinline__ Real end(const IntegrandConsts&, int, bool& pass) { pass = true; return f; }
+};
+
+// ------------------------------------------------------------------------------------------------
+// One event, S1-S4.  D = compile-time dimension (0: run-time a.dim), NB = compile-time bin count (0:
+// run-time a.nbins).  `tab` points to the staged table in shared memory, cell (k, i) at
+// tab[(k*N + i) * TSTRIDE + toff] (TSTRIDE/toff implement lane-replicated bank-conflict-free copies).
+// bins[] receives the d bin indices.  Returns wf = (double)J * (double)f.
+// ------------------------------------------------------------------------------------------------
+template <class F, int D, int NB>
+struct EventOut {
+    double wf;
+    bool pass;
+};
+
+template <class F, int D, int NB, int TSTRIDE, class BinSink>
+__device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
+                                                BinSink&& sink, typename F::real& J_out,
+                                                typename F::real& f_out, bool& pass)
+{
+    using real = typename F::real;
+    constexpr bool kF64 = (sizeof(real) == 8);
+    const int d = D ? D : a.dim;
+    const uint32_t N = NB ? static_cast<uint32_t>(NB) : static_cast<uint32_t>(a.nbins);
+    F integrand;
+    integrand.begin(a.ic);
+    real J = real(1);
+    uint32_t r[4] = {0u, 0u, 0u, 0u};
+    if constexpr (kF64) {
+        const double2* tab = static_cast<const double2*>(tab_);
+        const double Nd = static_cast<double>(N);
+#pragma unroll
+        for (int k = 0; k < (D ? D : kMaxDim); ++k) {
+            if (!D && k >= d) break;
+            if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 1), a, r);
+            const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
+            int i; double frac;
+            bin_frac64(w_lo, w_hi, N, i, frac);
+            const double2 t = tab[(k * static_cast<int>(N) + i) * TSTRIDE + toff];
+            const double x = __fma_rn(frac, t.y, t.x);
+            const double g = __dmul_rn(Nd, t.y);
+            J = (k == 0) ? g : __dmul_rn(J, g);
+            sink(k, i, x);
+            integrand.coord(k, x, a.ic);
+        }
+    } else {
+        const float2* tab = static_cast<const float2*>(tab_);
+        const float Nf = static_cast<float>(N);
+#pragma unroll
+        for (int k = 0; k < (D ? D : kMaxDim); ++k) {
+            if (!D && k >= d) break;
+            if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 2), a, r);
+            const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
+            int i; float frac;
+            bin_frac32(w, N, i, frac);
+            const float2 t = tab[(k * static_cast<int>(N) + i) * TSTRIDE + toff];
+            const float x = __fmaf_rn(frac, t.y, t.x);
+            const float g = __fmul_rn(Nf, t.y);
+            J = (k == 0) ? g : __fmul_rn(J, g);
+            sink(k, i, x);
+            integrand.coord(k, x, a.ic);
+        }
+    }
+    const real f = integrand.end(a.ic, d, pass);
+    J_out = J;
+    f_out = f;
+    return __dmul_rn(static_cast<double>(J), static_cast<double>(f));   // S4
+}
+
+}  // namespace vegas

@@ -1,0 +1,361 @@
+// vegas_kernels.cuh -- the kernels of the Vegas hot path (sm_100a): iterate (S1-S5), finalize (S6),
+// refine (S7), table staging and the per-event parity hook.  Steps and readings: DESIGN.md /
+// SURVEY.md 8.c; BASELINE.json north_star names the subsystems (event generation, grid mapping,
+// integrand evaluation, reduction, grid refinement, batching).  No code is shared with oracle/.
+#pragma once
+#include "vegas_device.cuh"
+
+namespace vegas {
+
+// ------------------------------------------------------------------------------------------------
+// Error-free transformations for the compensated sums (S5: "Kahan-compensated in FP64").
+// A compensated value is a pair (hi, lo) standing for hi + lo.
+// ------------------------------------------------------------------------------------------------
+struct Comp {
+    double hi, lo;
+};
+
+__device__ __forceinline__ void two_sum(double a, double b, double& s, double& r)
+{
+    s = __dadd_rn(a, b);
+    const double bb = __dsub_rn(s, a);
+    r = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
+}
+
+// Kahan step: add x to (hi, lo).  lo carries the rounding error of the running sum.
+__device__ __forceinline__ void kahan_add(Comp& c, double x)
+{
+    const double y = __dadd_rn(x, c.lo);
+    const double t = __dadd_rn(c.hi, y);
+    c.lo = __dsub_rn(y, __dsub_rn(t, c.hi));
+    c.hi = t;
+}
+
+// (hi, lo) += (ohi, olo), exact in the leading term.
+__device__ __forceinline__ void comp_add(Comp& c, double ohi, double olo)
+{
+    double s, r;
+    two_sum(c.hi, ohi, s, r);
+    c.hi = s;
+    c.lo = __dadd_rn(__dadd_rn(c.lo, olo), r);
+}
+
+__device__ __forceinline__ void comp_warp_reduce(Comp& c)
+{
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const double ohi = __shfl_down_sync(0xFFFFFFFFu, c.hi, off);
+        const double olo = __shfl_down_sync(0xFFFFFFFFu, c.lo, off);
+        comp_add(c, ohi, olo);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// iterate_kernel: S1-S5 for the events [e_first, e_first + count) of one launch.
+//
+// One thread owns whole events (all d coordinates): Philox words, mantissas, bins, x, J and f stay in
+// registers; the only memory traffic per event is d reads of the (lo, wd) table and d fp64 updates of
+// the histogram, both in shared memory.  HBM: one table read per CTA at entry, one d*N flush per CTA
+// at exit (global fp64 reductions), four doubles per CTA for the scalar sums.
+//
+// Shared memory:  hist[d*N][R] fp64 (R = 2^rshift lane-indexed replicas: lane l updates replica l%R, so
+//                 with R = 32 no two lanes of a warp ever touch the same word and the compare-and-swap
+//                 that fp64 shared atomics compile to on sm_100a succeeds first try unless another
+//                 warp got in between) | table[d*N] real2 | per-warp partial sums.
+// Grid: a multiple of the SM count; the events of the launch are dealt round-robin to threads
+// (idx = blockIdx*blockDim + tid, stride gridDim*blockDim), so the Philox counter of a thread's next
+// event is its previous one plus a constant.
+// ------------------------------------------------------------------------------------------------
+template <int D>
+struct BinPack {   // d bin indices, 16 bits each, kept in registers (all indices are compile-time)
+    uint32_t w[((D ? D : kMaxDim) + 1) / 2];
+    __device__ __forceinline__ void clear()
+    {
+#pragma unroll
+        for (int i = 0; i < ((D ? D : kMaxDim) + 1) / 2; ++i) w[i] = 0u;
+    }
+    __device__ __forceinline__ void set(int k, int i) { w[k >> 1] |= static_cast<uint32_t>(i) << ((k & 1) * 16); }
+    __device__ __forceinline__ int get(int k) const { return static_cast<int>((w[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu); }
+};
+
+template <class F, int D, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
+{
+    using real = typename F::real;
+    using real2 = typename std::conditional<sizeof(real) == 8, double2, float2>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+
+    const int d = D ? D : a.dim;
+    const int N = a.nbins;
+    const int cells = d * N;
+    const int R = 1 << a.rshift;
+    double* sh_hist = reinterpret_cast<double*>(smem_raw);
+    real2* sh_tab = reinterpret_cast<real2*>(smem_raw + static_cast<size_t>(cells) * R * sizeof(double));
+    double* sh_part = reinterpret_cast<double*>(smem_raw + static_cast<size_t>(cells) * R * sizeof(double) +
+                                                ((static_cast<size_t>(cells) * sizeof(real2) + 15) & ~size_t(15)));
+
+    const int tid = threadIdx.x;
+    const int lane = tid & 31;
+    for (int i = tid; i < cells * R; i += blockDim.x) sh_hist[i] = 0.0;
+    {
+        const real2* gt = static_cast<const real2*>(a.table);
+        for (int i = tid; i < cells; i += blockDim.x) sh_tab[i] = gt[i];
+    }
+    __syncthreads();
+
+    const int rep = lane & (R - 1);
+    Comp s1{0.0, 0.0}, s2{0.0, 0.0};
+    unsigned int np = 0;
+
+    const uint32_t stride = gridDim.x * blockDim.x;
+    for (uint32_t idx = blockIdx.x * blockDim.x + tid; idx < a.count; idx += stride) {
+        BinPack<D> bp;
+        bp.clear();
+        real J, f;
+        bool pass;
+        const double wf = process_event<F, D, 0, 1>(
+            a, a.e_lo_first + idx, sh_tab, 0, [&](int k, int i, real) { bp.set(k, i); }, J, f, pass);
+        const double q = __dmul_rn(wf, wf);                       // S4
+        kahan_add(s1, wf);                                        // S5
+        kahan_add(s2, q);
+        np += pass ? 1u : 0u;
+        if (q != 0.0) {                                           // adding 0 is the identity (reading R8)
+#pragma unroll
+            for (int k = 0; k < (D ? D : kMaxDim); ++k) {
+                if (!D && k >= d) break;
+                atomicAdd(&sh_hist[((k * N + bp.get(k)) << a.rshift) + rep], q);
+            }
+        }
+    }
+
+    // ---- scalar sums: warp shuffle tree on compensated pairs, then one thread per CTA ----
+    comp_warp_reduce(s1);
+    comp_warp_reduce(s2);
+    np = __reduce_add_sync(0xFFFFFFFFu, np);
+    const int warp = tid >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if (lane == 0) {
+        sh_part[warp * 5 + 0] = s1.hi; sh_part[warp * 5 + 1] = s1.lo;
+        sh_part[warp * 5 + 2] = s2.hi; sh_part[warp * 5 + 3] = s2.lo;
+        sh_part[warp * 5 + 4] = static_cast<double>(np);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        // the CTA's slot carries over from the previous launches of this iteration (stream order)
+        double* slot = a.slots + static_cast<size_t>(blockIdx.x) * 4;
+        Comp t1{slot[0], slot[1]}, t2{slot[2], slot[3]};
+        unsigned long long npb = 0;
+        for (int w = 0; w < nwarps; ++w) {
+            comp_add(t1, sh_part[w * 5 + 0], sh_part[w * 5 + 1]);
+            comp_add(t2, sh_part[w * 5 + 2], sh_part[w * 5 + 3]);
+            npb += static_cast<unsigned long long>(sh_part[w * 5 + 4]);
+        }
+        slot[0] = t1.hi; slot[1] = t1.lo; slot[2] = t2.hi; slot[3] = t2.lo;
+        if (npb) atomicAdd(a.npass, npb);
+    }
+
+    // ---- histogram flush: fixed-order sum over the replicas, one global reduction per touched cell ----
+    for (int c = tid; c < cells; c += blockDim.x) {
+        const double* p = sh_hist + (static_cast<size_t>(c) << a.rshift);
+        double v = p[0];
+        for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[r]);
+        if (v != 0.0) atomicAdd(a.hist + c, v);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// finalize_kernel (S6): fixed-order compensated sum of the per-CTA slots, then
+//   I = S1/n ; V = (S2/n - I*I)/(n-1) ; sigma = sqrt(max(V, 0)).
+// One warp; lane l folds slots l, l+32, ... then a shuffle tree: the order depends only on nslots.
+// result[0..5] = I, sigma, S1, S2, npass, n
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__ slots, int nslots,
+                                                      const unsigned long long* __restrict__ npass,
+                                                      unsigned long long n_events, double* __restrict__ result)
+{
+    const int lane = threadIdx.x;
+    Comp t1{0.0, 0.0}, t2{0.0, 0.0};
+    for (int s = lane; s < nslots; s += 32) {
+        comp_add(t1, slots[s * 4 + 0], slots[s * 4 + 1]);
+        comp_add(t2, slots[s * 4 + 2], slots[s * 4 + 3]);
+    }
+    comp_warp_reduce(t1);
+    comp_warp_reduce(t2);
+    if (lane == 0) {
+        const double S1 = __dadd_rn(t1.hi, t1.lo), S2 = __dadd_rn(t2.hi, t2.lo);
+        const double n = static_cast<double>(n_events);
+        const double I = __ddiv_rn(S1, n);
+        const double V = __ddiv_rn(__dsub_rn(__ddiv_rn(S2, n), __dmul_rn(I, I)), __dsub_rn(n, 1.0));
+        result[0] = I;
+        result[1] = sqrt(V > 0.0 ? V : 0.0);
+        result[2] = S1;
+        result[3] = S2;
+        result[4] = static_cast<double>(*npass);
+        result[5] = n;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Grid state kernels.  Master edges E[d][N+1] are fp64; the mapping table holds (lo, wd) per cell in the
+// working precision (S2):  uniform grid: lo = rnd(E[i]), wd = rnd(fl64(1/N));
+//                          otherwise:    lo = rnd(E[i]), wd = rnd(fl64(E[i+1]-E[i])).
+// g = fl(N*wd) is recomputed per event from wd (one multiply; same bits as a stored g).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void write_table_cell(void* table, int precision, size_t cell, double lo, double wd)
+{
+    if (precision == 0) static_cast<double2*>(table)[cell] = make_double2(lo, wd);
+    else static_cast<float2*>(table)[cell] = make_float2(__double2float_rn(lo), __double2float_rn(wd));
+}
+
+// one CTA per dimension.  uniform != 0: also (re)writes E[k][i] = fl64(i/N), E[k][N] = 1.
+__global__ void build_table_kernel(double* __restrict__ edges, void* __restrict__ table, int N, int precision,
+                                   int uniform)
+{
+    const int k = blockIdx.x;
+    double* E = edges + static_cast<size_t>(k) * (N + 1);
+    if (uniform) {
+        const double Nd = static_cast<double>(N);
+        for (int i = threadIdx.x; i <= N; i += blockDim.x) E[i] = (i == N) ? 1.0 : __ddiv_rn(static_cast<double>(i), Nd);
+        __syncthreads();
+        const double wd = __ddiv_rn(1.0, Nd);
+        for (int i = threadIdx.x; i < N; i += blockDim.x)
+            write_table_cell(table, precision, static_cast<size_t>(k) * N + i, E[i], wd);
+    } else {
+        for (int i = threadIdx.x; i < N; i += blockDim.x)
+            write_table_cell(table, precision, static_cast<size_t>(k) * N + i, E[i], __dsub_rn(E[i + 1], E[i]));
+    }
+}
+
+// refine_kernel (S7, steps 1-6 + the monotonicity check of step 7): one CTA per dimension.  Sums and
+// prefix sums are sequential in ascending i (one thread), exactly the order the definition states; the
+// per-bin work (smoothing, damping, edge interpolation) is spread over the threads.
+//   new_edges[k][*] receives the candidate edges; flags[k] = 0 ok / 1 not strictly increasing.
+__global__ void refine_kernel(const double* __restrict__ edges, const double* __restrict__ hist, int N,
+                              double alpha, double* __restrict__ new_edges, int* __restrict__ flags)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double* s = reinterpret_cast<double*>(smem_raw);   // [N]   smoothed
+    double* m = s + N;                                  // [N]   damped weights
+    double* cum = m + N;                                // [N+1] prefix sums
+    __shared__ double sh_scalar;
+    __shared__ int sh_bad;
+
+    const int k = blockIdx.x, tid = threadIdx.x;
+    const double* h = hist + static_cast<size_t>(k) * N;
+    const double* E = edges + static_cast<size_t>(k) * (N + 1);
+    double* En = new_edges + static_cast<size_t>(k) * (N + 1);
+
+    if (tid == 0) {                                     // step 1
+        double tot = 0.0;
+        for (int i = 0; i < N; ++i) tot = __dadd_rn(tot, h[i]);
+        sh_scalar = tot;
+        sh_bad = 0;
+    }
+    __syncthreads();
+    const double tot = sh_scalar;
+    if (!(tot > 0.0) || !isfinite(tot)) {               // nothing to adapt to: dimension unchanged
+        for (int i = tid; i <= N; i += blockDim.x) En[i] = E[i];
+        if (tid == 0) flags[k] = 0;
+        return;
+    }
+    for (int i = tid; i < N; i += blockDim.x) {         // step 2
+        double v;
+        if (i == 0) v = __ddiv_rn(__dadd_rn(h[0], h[1]), 2.0);
+        else if (i == N - 1) v = __ddiv_rn(__dadd_rn(h[N - 2], h[N - 1]), 2.0);
+        else v = __ddiv_rn(__dadd_rn(__dadd_rn(h[i - 1], h[i]), h[i + 1]), 3.0);
+        s[i] = v;
+    }
+    __syncthreads();
+    if (tid == 0) {                                     // step 3
+        double ssum = 0.0;
+        for (int i = 0; i < N; ++i) ssum = __dadd_rn(ssum, s[i]);
+        sh_scalar = ssum;
+    }
+    __syncthreads();
+    const double ssum = sh_scalar;
+    for (int i = tid; i < N; i += blockDim.x) {         // step 4
+        const double r = __ddiv_rn(s[i], ssum);
+        double v;
+        if (r <= 0.0) v = 0.0;
+        else if (r >= 1.0) v = 1.0;
+        else v = pow(__ddiv_rn(__dsub_rn(1.0, r), -log(r)), alpha);
+        m[i] = v;
+    }
+    __syncthreads();
+    if (tid == 0) {                                     // step 5
+        double c = 0.0;
+        cum[0] = 0.0;
+        for (int i = 0; i < N; ++i) { c = __dadd_rn(c, m[i]); cum[i + 1] = c; }
+        sh_scalar = __ddiv_rn(c, static_cast<double>(N));
+    }
+    __syncthreads();
+    const double delta = sh_scalar;
+    for (int j = tid; j <= N; j += blockDim.x) {        // step 6
+        double v;
+        if (j == 0) v = 0.0;
+        else if (j == N) v = 1.0;
+        else {
+            const double t = __dmul_rn(static_cast<double>(j), delta);
+            int i = 0;
+            while (i < N - 1 && !(cum[i + 1] >= t && m[i] > 0.0)) ++i;
+            v = __dadd_rn(E[i], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[i]), m[i]), __dsub_rn(E[i + 1], E[i])));
+        }
+        En[j] = v;
+    }
+    __syncthreads();
+    for (int j = tid; j < N; j += blockDim.x)           // step 7 check
+        if (!(En[j] < En[j + 1])) sh_bad = 1;
+    __syncthreads();
+    if (tid == 0) flags[k] = sh_bad;
+}
+
+// commit (S7 step 7): if every dimension passed, the candidate edges become the master edges, the table
+// is rebuilt and H is cleared; otherwise nothing changes.  status[0] = 0 ok / 1 rejected.
+__global__ void refine_commit_kernel(double* __restrict__ edges, const double* __restrict__ new_edges,
+                                     const int* __restrict__ flags, int d, int N, void* __restrict__ table,
+                                     int precision, double* __restrict__ hist, int* __restrict__ status)
+{
+    const int k = blockIdx.x;
+    int bad = 0;
+    for (int j = 0; j < d; ++j) bad |= flags[j];
+    if (threadIdx.x == 0 && k == 0) status[0] = bad;
+    if (bad) return;
+    double* E = edges + static_cast<size_t>(k) * (N + 1);
+    const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
+    for (int i = threadIdx.x; i < N; i += blockDim.x) {
+        const double lo = En[i], hi = En[i + 1];
+        write_table_cell(table, precision, static_cast<size_t>(k) * N + i, lo, __dsub_rn(hi, lo));
+        hist[static_cast<size_t>(k) * N + i] = 0.0;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i <= N; i += blockDim.x) E[i] = En[i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// debug_events_kernel: the parity hook.  One thread per event, same process_event as iterate_kernel,
+// table read from global memory.
+// ------------------------------------------------------------------------------------------------
+template <class F, int D>
+__global__ void debug_events_kernel(const __grid_constant__ IterArgs a, int32_t* __restrict__ bins,
+                                    double* __restrict__ x, double* __restrict__ jac, double* __restrict__ f,
+                                    double* __restrict__ wf, int32_t* __restrict__ pass)
+{
+    using real = typename F::real;
+    const uint32_t idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= a.count) return;
+    const int d = D ? D : a.dim;
+    real J, fv;
+    bool ps;
+    const double w = process_event<F, D, 0, 1>(
+        a, a.e_lo_first + idx, a.table, 0,
+        [&](int k, int i, real xv) {
+            bins[static_cast<size_t>(idx) * d + k] = i;
+            x[static_cast<size_t>(idx) * d + k] = static_cast<double>(xv);
+        },
+        J, fv, ps);
+    jac[idx] = static_cast<double>(J);
+    f[idx] = static_cast<double>(fv);
+    wf[idx] = w;
+    pass[idx] = ps ? 1 : 0;
+}
+
+}  // namespace vegas

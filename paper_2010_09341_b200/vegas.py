@@ -1,0 +1,206 @@
+"""ctypes binding of libvegas_b200.so -- same names as include/vegas_b200.h, argument marshalling only.
+
+Every step of the path (S1-S7) runs in the library's CUDA kernels.  PyTorch supplies the device
+workspace (``torch.empty(..., dtype=uint8, device='cuda')``) and the stream
+(``torch.cuda.current_stream().cuda_stream``), nothing else.  If the library cannot be built/loaded or
+there is no CUDA device, calls raise: there is no CPU fallback.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+OK, EINVAL, ECUDA, ENOMEM, ESTATE, EUNSUPPORTED, EGRID = 0, -1, -2, -3, -4, -5, -6
+FP64, FP32_EVAL = 0, 1
+GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM = 0, 1, 2, 3, 4
+
+_vp, _dp, _ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+_i32p, _u32p, _u64p, _szp = C.POINTER(C.c_int32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_size_t)
+
+# name -> (restype, argtypes): every symbol include/vegas_b200.h declares
+SIGNATURES = {
+    "vegas_workspace_bytes": (C.c_size_t, [C.c_int, C.c_int]),
+    "vegas_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
+    "vegas_iterate": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp, _dp]),
+    "vegas_refine": (C.c_int, [_vp, C.c_double]),
+    "vegas_get_grid": (C.c_int, [_vp, _dp]),
+    "vegas_set_grid": (C.c_int, [_vp, _dp]),
+    "vegas_reset": (C.c_int, [_vp]),
+    "vegas_set_iteration": (C.c_int, [_vp, C.c_uint32]),
+    "vegas_get_iteration": (C.c_int, [_vp, _u32p]),
+    "vegas_debug_events": (C.c_int, [_vp, C.c_uint64, C.c_uint32, C.c_uint64, _i32p, _dp, _dp, _dp, _dp, _i32p]),
+    "vegas_last_sums": (C.c_int, [_vp, _dp, _dp, _dp]),
+    "vegas_last_npass": (C.c_int, [_vp, _u64p]),
+    "vegas_iterate_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _ip]),
+    "vegas_iterate_collect": (C.c_int, [_vp, _dp, _dp, _dp]),
+    "vegas_set_launch_shape": (C.c_int, [_vp, C.c_int, C.c_int]),
+    "vegas_set_hist_replicas": (C.c_int, [_vp, C.c_int]),
+    "vegas_get_launch_shape": (C.c_int, [_vp, _ip, _ip, _ip, _szp]),
+    "vegas_device_info": (C.c_int, [_vp, _ip, _ip]),
+    "vegas_destroy": (None, [_vp]),
+    "vegas_last_error": (C.c_char_p, []),
+}
+
+_lib = None
+
+
+def lib():
+    """Load (building first if the sources are newer) libvegas_b200.so.  Raises if that fails."""
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)          # AttributeError if the library does not export it
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+class VegasError(RuntimeError):
+    def __init__(self, code, what):
+        msg = lib().vegas_last_error()
+        super().__init__("%s failed with status %d: %s" % (what, code, msg.decode() if msg else ""))
+        self.code = code
+
+
+def _chk(code, what):
+    if code != OK:
+        raise VegasError(code, what)
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp)
+
+
+def workspace_bytes(dim, nbins):
+    return int(lib().vegas_workspace_bytes(dim, nbins))
+
+
+class Vegas:
+    """One integrator state on the GPU: VegasFlow(n_dim, ...) + compile(integrand) of PAPER.md:L77-L78."""
+
+    def __init__(self, dim, nbins, integrand_id, params=(), precision=FP64, stream=None, device="cuda:0"):
+        import torch  # device memory and stream only
+
+        L = lib()
+        self._h = None
+        nbytes = workspace_bytes(dim, nbins)
+        p = np.ascontiguousarray(np.asarray(params, dtype=np.float64))
+        if nbytes == 0 or not torch.cuda.is_available():
+            # let the library report the error (EINVAL ranges first, then ECUDA: no CPU fallback)
+            h = _vp()
+            rc = L.vegas_create(C.byref(h), dim, nbins, integrand_id, _d(p) if p.size else None, int(p.size),
+                                precision, None if nbytes == 0 else _vp(256), max(nbytes, 1), None)
+            raise VegasError(rc if rc != OK else ECUDA, "vegas_create")
+        self._dev = torch.device(device)
+        torch.cuda.set_device(self._dev)
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self._dev)
+        ptr = (self._ws.data_ptr() + 255) & ~255
+        self._stream = stream if stream is not None else torch.cuda.current_stream(self._dev)
+        h = _vp()
+        _chk(L.vegas_create(C.byref(h), dim, nbins, integrand_id, _d(p) if p.size else None, int(p.size), precision,
+                            _vp(ptr), nbytes, _vp(self._stream.cuda_stream)), "vegas_create")
+        self._h = h
+        self.dim, self.nbins, self.integrand_id, self.precision = dim, nbins, integrand_id, precision
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().vegas_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    # ---- the three calls of BASELINE.json north_star ------------------------------------------------
+    def iterate(self, n_events, events_per_launch=0, seed=0, want_hist=True):
+        n_events = int(n_events)
+        epl = int(events_per_launch) if events_per_launch else n_events
+        I, s = C.c_double(), C.c_double()
+        h = np.empty((self.dim, self.nbins)) if want_hist else None
+        _chk(lib().vegas_iterate(self._h, n_events, epl, int(seed), C.byref(I), C.byref(s),
+                                 _d(h) if want_hist else None), "vegas_iterate")
+        return I.value, s.value, h
+
+    def refine(self, alpha):
+        _chk(lib().vegas_refine(self._h, float(alpha)), "vegas_refine")
+
+    # ---- asynchronous form (timing) ------------------------------------------------------------------
+    def iterate_enqueue(self, n_events, events_per_launch=0, seed=0):
+        n_events = int(n_events)
+        epl = int(events_per_launch) if events_per_launch else n_events
+        nl = C.c_int()
+        _chk(lib().vegas_iterate_enqueue(self._h, n_events, epl, int(seed), C.byref(nl)), "vegas_iterate_enqueue")
+        return nl.value
+
+    def iterate_collect(self, want_hist=True):
+        I, s = C.c_double(), C.c_double()
+        h = np.empty((self.dim, self.nbins)) if want_hist else None
+        _chk(lib().vegas_iterate_collect(self._h, C.byref(I), C.byref(s), _d(h) if want_hist else None),
+             "vegas_iterate_collect")
+        return I.value, s.value, h
+
+    # ---- state ---------------------------------------------------------------------------------------
+    def get_grid(self):
+        e = np.empty((self.dim, self.nbins + 1))
+        _chk(lib().vegas_get_grid(self._h, _d(e)), "vegas_get_grid")
+        return e
+
+    def set_grid(self, edges):
+        e = np.ascontiguousarray(edges, dtype=np.float64)
+        assert e.shape == (self.dim, self.nbins + 1)
+        _chk(lib().vegas_set_grid(self._h, _d(e)), "vegas_set_grid")
+
+    def reset(self):
+        _chk(lib().vegas_reset(self._h), "vegas_reset")
+
+    def set_iteration(self, it):
+        _chk(lib().vegas_set_iteration(self._h, int(it)), "vegas_set_iteration")
+
+    @property
+    def iteration(self):
+        v = C.c_uint32()
+        _chk(lib().vegas_get_iteration(self._h, C.byref(v)), "vegas_get_iteration")
+        return v.value
+
+    def debug_events(self, first, count, seed=0):
+        d = self.dim
+        bins = np.empty((count, d), dtype=np.int32)
+        x = np.empty((count, d)); jac = np.empty(count); f = np.empty(count); wf = np.empty(count)
+        ps = np.empty(count, dtype=np.int32)
+        _chk(lib().vegas_debug_events(self._h, int(first), int(count), int(seed), bins.ctypes.data_as(_i32p), _d(x),
+                                      _d(jac), _d(f), _d(wf), ps.ctypes.data_as(_i32p)), "vegas_debug_events")
+        return dict(bins=bins, x=x, jac=jac, f=f, wf=wf, passed=ps)
+
+    def last_sums(self):
+        a, b, ms = C.c_double(), C.c_double(), C.c_double()
+        _chk(lib().vegas_last_sums(self._h, C.byref(a), C.byref(b), C.byref(ms)), "vegas_last_sums")
+        return a.value, b.value, ms.value
+
+    def last_npass(self):
+        v = C.c_uint64()
+        _chk(lib().vegas_last_npass(self._h, C.byref(v)), "vegas_last_npass")
+        return v.value
+
+    def set_launch_shape(self, ctas_per_sm=0, threads_per_cta=0):
+        _chk(lib().vegas_set_launch_shape(self._h, ctas_per_sm, threads_per_cta), "vegas_set_launch_shape")
+
+    def set_hist_replicas(self, replicas=0):
+        _chk(lib().vegas_set_hist_replicas(self._h, replicas), "vegas_set_hist_replicas")
+
+    def launch_shape(self):
+        a, b, r, s = C.c_int(), C.c_int(), C.c_int(), C.c_size_t()
+        _chk(lib().vegas_get_launch_shape(self._h, C.byref(a), C.byref(b), C.byref(r), C.byref(s)),
+             "vegas_get_launch_shape")
+        return dict(ctas_per_sm=a.value, threads_per_cta=b.value, hist_replicas=r.value, smem_bytes=s.value)
+
+    def device_info(self):
+        a, b = C.c_int(), C.c_int()
+        _chk(lib().vegas_device_info(self._h, C.byref(a), C.byref(b)), "vegas_device_info")
+        return dict(sm_count=a.value, sm_clock_khz=b.value)
+
+
+def from_workload(w, **kw):
+    """Vegas(...) for a paper_2010_09341_b200.workloads.Workload."""
+    return Vegas(w.dim, w.nbins, w.integrand_id, w.params, w.precision, **kw)

@@ -1,0 +1,303 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances are those of BASELINE.json north_star: bins / pass / mapped point bit-exact,
+I and sigma rel 1e-12, histogram rel 1e-10 per cell (zero cells zero on both sides), refined edges abs
+1e-12 after 5 iterations.  Per-event integrand values: bit-exact where the arithmetic is fully specified
+(fp32 genz_osc_peak, toy_sum), a few ulp where a libm exp() is involved (glibc vs CUDA).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2010_09341_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+THREADS = max(1, min(32, len(os.sched_getaffinity(0))))
+
+
+@pytest.fixture(scope="module")
+def V():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2010_09341_b200 import vegas
+    return vegas
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    return oracle
+
+
+def small_workloads():
+    return {
+        "cfg1": W.cfg1(), "cfg2": W.cfg2(), "cfg4": W.cfg4(), "cfg5": W.cfg5(), "toy": W.toy(),
+        # run-time-dimension instances
+        "gauss_sym_d2": W.Workload("gs2", 2, 37, W.GAUSS_SYM, (0.1, 0.5), W.FP64, 10**5, 3),
+        "gauss_double_d5": W.Workload("gd5", 5, 64, W.GAUSS_DOUBLE, (0.1, 1 / 3, 2 / 3), W.FP64, 10**5, 3),
+        "genz_d7": W.cfg4(dim=7),
+        "toy_d32": W.Workload("toy32", 32, 50, W.TOY_SUM, (), W.FP64, 10**5, 3),
+        "toy_f32_d9": W.Workload("toyf9", 9, 100, W.TOY_SUM, (), W.FP32_EVAL, 10**5, 3),
+    }
+
+
+F_RTOL = {W.GAUSS_SYM: 2e-15, W.GAUSS_DOUBLE: 2e-15, W.GENZ_OSC_PEAK: 0.0, W.LO_2TO2: 2e-14, W.TOY_SUM: 0.0}
+
+
+def make_pair(V, O, w):
+    return V.from_workload(w), O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+
+
+def assert_events_equal(g, o, w):
+    np.testing.assert_array_equal(g["bins"], o["bins"])
+    np.testing.assert_array_equal(g["passed"], o["passed"])
+    np.testing.assert_array_equal(g["x"], o["x"])            # bit-exact mapped point (S2)
+    np.testing.assert_array_equal(g["jac"], o["jac"])
+    rt = F_RTOL[w.integrand_id]
+    if rt == 0.0:
+        np.testing.assert_array_equal(g["f"], o["f"])
+        np.testing.assert_array_equal(g["wf"], o["wf"])
+    else:
+        np.testing.assert_allclose(g["f"], o["f"], rtol=rt, atol=0.0)
+        np.testing.assert_allclose(g["wf"], o["wf"], rtol=rt, atol=0.0)
+
+
+def assert_iteration_close(gres, ores):
+    gI, gs, gh = gres
+    oI, os_, oh = ores
+    assert abs(gI - oI) <= 1e-12 * abs(oI), (gI, oI)
+    assert abs(gs - os_) <= 1e-12 * abs(os_), (gs, os_)
+    assert np.array_equal(gh == 0.0, oh == 0.0)
+    np.testing.assert_allclose(gh, oh, rtol=1e-10, atol=0.0)
+
+
+# ---------------------------------------------------------------------------------------------------
+# per-event parity (S1-S4)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", list(small_workloads()))
+def test_events_uniform_grid(V, O, name):
+    w = small_workloads()[name]
+    g, o = make_pair(V, O, w)
+    for first, count in [(0, 5000), (99_990_000, 777), (2**32 - 300, 300), (2**32, 129), (2**40 + 12345, 64)]:
+        assert_events_equal(g.debug_events(first, count, seed=w.seed), o.events(first, count, w.seed), w)
+    # another seed and iteration counter
+    g.set_iteration(7); o.set_iteration(7)
+    assert_events_equal(g.debug_events(1000, 2000, seed=0xDEADBEEF12345678), o.events(1000, 2000, 0xDEADBEEF12345678), w)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg4", "cfg5", "gauss_double_d5"])
+def test_events_adapted_grid(V, O, name):
+    """Cascade-free: load the oracle's refined grid into the library, then compare events."""
+    w = small_workloads()[name]
+    g, o = make_pair(V, O, w)
+    for _ in range(2):
+        o.iterate(200_000, w.seed, threads=THREADS)
+        o.refine(w.alpha)
+    g.set_grid(o.get_grid())
+    g.set_iteration(o.iteration)
+    np.testing.assert_array_equal(g.get_grid(), o.get_grid())
+    assert_events_equal(g.debug_events(0, 20_000, seed=w.seed), o.events(0, 20_000, w.seed), w)
+    if w.integrand_id not in (W.TOY_SUM,):
+        assert np.any(o.events(0, 100, w.seed)["jac"] != 1.0)
+
+
+# ---------------------------------------------------------------------------------------------------
+# one iteration (S1-S6): several tiles + a ragged tail, several launch splits
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", list(small_workloads()))
+def test_iteration_parity(V, O, name):
+    w = small_workloads()[name]
+    g, o = make_pair(V, O, w)
+    n = 1_000_003
+    ores = o.iterate(n, w.seed, threads=THREADS)
+    for epl in (0, 65_537, 300_000):
+        g.reset()
+        gres = g.iterate(n, epl, w.seed)
+        assert_iteration_close(gres, ores)
+        S1, S2, _ = g.last_sums()
+        oS1, oS2 = o.last_sums()
+        assert abs(S1 - oS1) <= 1e-12 * abs(oS1) and abs(S2 - oS2) <= 1e-12 * abs(oS2)
+        # invariant P4: every dimension's histogram sums to S2
+        np.testing.assert_allclose(gres[2].sum(axis=1), S2, rtol=1e-12)
+    if o.npass is not None:
+        assert g.last_npass() == o.npass
+
+
+def test_iteration_launch_shapes(V, O):
+    """Results do not depend on the launch shape or replica count beyond summation order."""
+    w = W.cfg2()
+    g, o = make_pair(V, O, w)
+    n = 500_009
+    ores = o.iterate(n, 3, threads=THREADS)
+    for ctas, threads, reps in [(1, 1024, 32), (2, 512, 16), (4, 256, 8), (1, 128, 1), (8, 64, 2)]:
+        g.reset()
+        g.set_launch_shape(ctas, threads)
+        g.set_hist_replicas(reps)
+        assert g.launch_shape()["hist_replicas"] == reps
+        assert_iteration_close(g.iterate(n, 0, 3), ores)
+
+
+def test_batch_size_independence(V):
+    """Reading R16: the event index is global, so events_per_launch changes nothing but summation order."""
+    w = W.cfg2()
+    g = V.from_workload(w)
+    ref = None
+    for epl in (10**4, 10**5, 10**6, 2 * 10**6):
+        g.reset()
+        I, s, h = g.iterate(2 * 10**6, epl, 0)
+        if ref is None:
+            ref = (I, s, h)
+        assert abs(I - ref[0]) <= 1e-13 * abs(ref[0]) and abs(s - ref[1]) <= 1e-13 * abs(ref[1])
+        np.testing.assert_allclose(h, ref[2], rtol=1e-12)
+
+
+# ---------------------------------------------------------------------------------------------------
+# iterate + refine cascades (S7)
+# ---------------------------------------------------------------------------------------------------
+def run_cascade(g, o, w, n, n_iter, epl=0):
+    for it in range(n_iter):
+        ores = o.iterate(n, w.seed, threads=THREADS)
+        gres = g.iterate(n, epl, w.seed)
+        assert_iteration_close(gres, ores)
+        o.refine(w.alpha)
+        g.refine(w.alpha)
+        ge, oe = g.get_grid(), o.get_grid()
+        assert np.all(np.diff(ge, axis=1) > 0) and np.all(ge[:, 0] == 0) and np.all(ge[:, -1] == 1)
+        assert np.max(np.abs(ge - oe)) <= 1e-12, (it, np.max(np.abs(ge - oe)))
+    assert g.iteration == o.iteration == n_iter
+
+
+def test_cfg1_full_five_iterations(V, O):
+    """BASELINE.json configs[0] at full size: 1e5 events x 5 iterations, alpha = 1.5, seed 0."""
+    w = W.cfg1()
+    g, o = make_pair(V, O, w)
+    run_cascade(g, o, w, w.n_events, w.n_iter)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "toy", "gauss_sym_d2", "toy_f32_d9"])
+def test_cascade_reduced(V, O, name):
+    w = small_workloads()[name]
+    g, o = make_pair(V, O, w)
+    run_cascade(g, o, w, 400_000, 5, epl=w.events_per_launch)
+
+
+def test_refine_alpha_zero_and_flat(V, O):
+    w = W.Workload("toy3", 3, 16, W.TOY_SUM, (), W.FP64, 10**5, 1)
+    g, o = make_pair(V, O, w)
+    o.iterate(50_000, 1); g.iterate(50_000, 0, 1)
+    o.refine(0.0); g.refine(0.0)
+    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-15
+    # alpha = 0: all damped weights are 1 -> the grid stays uniform
+    assert np.max(np.abs(g.get_grid() - np.linspace(0, 1, 17)[None, :])) <= 1e-15
+
+
+def test_all_events_cut_away(V, O):
+    """Degenerate: cos_cut = 0 rejects every event: I = sigma = 0, H = 0, refine leaves the grid unchanged."""
+    w = W.Workload("lo_cut", 3, 50, W.LO_2TO2, (13000.0, 50.0, 0.0, 1.1, 5.0), W.FP64, 10**5, 1)
+    g, o = make_pair(V, O, w)
+    I, s, h = g.iterate(100_000, 0, 0)
+    oI, os_, oh = o.iterate(100_000, 0)
+    assert I == oI == 0.0 and s == os_ == 0.0 and not h.any() and not oh.any()
+    assert g.last_npass() == 0
+    before = g.get_grid()
+    g.refine(1.5); o.refine(1.5)
+    np.testing.assert_array_equal(g.get_grid(), before)
+    np.testing.assert_array_equal(o.get_grid(), before)
+
+
+def test_extreme_sizes(V, O):
+    """Minimum n, one event per launch, maximum bin counts (fp64 4095, fp32 511), dim 32."""
+    w = W.Workload("toy1", 1, 4095, W.TOY_SUM, (), W.FP64, 10**5, 1)
+    g, o = make_pair(V, O, w)
+    assert_iteration_close(g.iterate(300_001, 0, 5), o.iterate(300_001, 5, threads=THREADS))
+    g.refine(1.5); o.refine(1.5)
+    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+    assert_events_equal(g.debug_events(0, 3000, 5), o.events(0, 3000, 5), w)
+
+    w = W.Workload("toyf", 2, 511, W.TOY_SUM, (), W.FP32_EVAL, 10**5, 1)
+    g, o = make_pair(V, O, w)
+    assert_iteration_close(g.iterate(200_001, 0, 5), o.iterate(200_001, 5, threads=THREADS))
+    g.refine(1.5); o.refine(1.5)
+    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+    assert_events_equal(g.debug_events(0, 3000, 5), o.events(0, 3000, 5), w)
+
+    w = W.cfg1()
+    g, o = make_pair(V, O, w)
+    assert_iteration_close(g.iterate(2, 0, 0), o.iterate(2, 0))
+    g.reset(); o.reset()
+    assert_iteration_close(g.iterate(64, 1, 0), o.iterate(64, 0))         # 64 launches of one event
+
+
+# ---------------------------------------------------------------------------------------------------
+# API state machine and error behaviour (include/vegas_b200.h)
+# ---------------------------------------------------------------------------------------------------
+def test_api_state_and_errors(V):
+    w = W.cfg1()
+    g = V.from_workload(w)
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(1.5)                                   # no histogram yet
+    assert ei.value.code == V.ESTATE
+    with pytest.raises(V.VegasError) as ei:
+        g.last_sums()
+    assert ei.value.code == V.ESTATE
+    with pytest.raises(V.VegasError) as ei:
+        g.iterate(1)
+    assert ei.value.code == V.EINVAL
+    g.iterate(10_000)
+    assert g.iteration == 1
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(-1.0)
+    assert ei.value.code == V.EINVAL
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(float("nan"))
+    assert ei.value.code == V.EINVAL
+    g.refine(1.5)
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(1.5)                                   # histogram was consumed
+    assert ei.value.code == V.ESTATE
+    e = g.get_grid()
+    g.set_grid(e)
+    np.testing.assert_array_equal(g.get_grid(), e)      # identity (P4)
+    bad = e.copy(); bad[1, 10] = bad[1, 11]
+    with pytest.raises(V.VegasError) as ei:
+        g.set_grid(bad)
+    assert ei.value.code == V.EGRID
+    np.testing.assert_array_equal(g.get_grid(), e)      # unchanged
+    bad = e.copy(); bad[0, -1] = 0.999
+    with pytest.raises(V.VegasError) as ei:
+        g.set_grid(bad)
+    assert ei.value.code == V.EGRID
+    g.reset()
+    assert g.iteration == 0
+    u = g.get_grid()
+    np.testing.assert_array_equal(u[0], np.array([i / 50 for i in range(50)] + [1.0]))
+    with pytest.raises(V.VegasError) as ei:
+        g.set_launch_shape(1, 100)
+    assert ei.value.code == V.EINVAL
+    info = g.device_info()
+    assert info["sm_count"] >= 100
+
+
+def test_uniform_grid_jacobian_is_one(V):
+    """P4 / reading R6: on the uniform grid J == 1 exactly for N = 50, 100."""
+    for w in (W.cfg2(), W.cfg4()):
+        g = V.from_workload(w)
+        ev = g.debug_events(0, 10_000, 0)
+        assert np.all(ev["jac"] == 1.0)
+        assert ev["bins"].min() >= 0 and ev["bins"].max() < w.nbins
+        assert np.all((ev["x"] >= 0) & (ev["x"] <= 1))
+
+
+def test_estimates_within_4_sigma_of_closed_form(V, golden_dir):
+    """P3 on the GPU path alone: adapted estimates land within 4 sigma of the exact integrals."""
+    from conftest import read_golden
+    exact = read_golden(os.path.join(golden_dir, "closed_forms.txt"))
+    for name, key in [("cfg1", "cfg1"), ("cfg5", "cfg5"), ("toy", None)]:
+        w = small_workloads()[name]
+        target = float(exact[key][0]) if key else w.dim / 2.0
+        g = V.from_workload(w)
+        for _ in range(6):
+            I, s, _ = g.iterate(10**6, 0, w.seed)
+            g.refine(w.alpha)
+        assert abs(I - target) <= 4 * s, (name, I, s)
