@@ -218,7 +218,7 @@ size_t iterate_smem_bytes(const vegas_ctx* c, int rshift, int threads)
 {
     const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
     const size_t cell_bytes = (c->precision == VEGAS_FP64) ? 16 : 8;
-    return cells * (size_t(1) << rshift) * 8 + align_up(cells * cell_bytes, 16) + static_cast<size_t>((threads + 31) / 32) * 5 * 8;
+    return align_up(cells * (size_t(1) << rshift) * 8, 16) + align_up(cells * cell_bytes, 16) + static_cast<size_t>((threads + 31) / 32) * 5 * 8;
 }
 
 // Choose R = 2^rshift: the largest power of two <= 32 such that `ctas` CTAs fit in the SM's shared memory.

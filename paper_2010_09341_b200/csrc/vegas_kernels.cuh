@@ -89,9 +89,10 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
     const int N = a.nbins;
     const int cells = d * N;
     const int R = 1 << a.rshift;
+    const size_t hist_bytes = (static_cast<size_t>(cells) * R * sizeof(double) + 15) & ~size_t(15);
     double* sh_hist = reinterpret_cast<double*>(smem_raw);
-    real2* sh_tab = reinterpret_cast<real2*>(smem_raw + static_cast<size_t>(cells) * R * sizeof(double));
-    double* sh_part = reinterpret_cast<double*>(smem_raw + static_cast<size_t>(cells) * R * sizeof(double) +
+    real2* sh_tab = reinterpret_cast<real2*>(smem_raw + hist_bytes);
+    double* sh_part = reinterpret_cast<double*>(smem_raw + hist_bytes +
                                                 ((static_cast<size_t>(cells) * sizeof(real2) + 15) & ~size_t(15)));
 
     const int tid = threadIdx.x;

@@ -213,6 +213,7 @@ def test_extreme_sizes(V, O):
     assert_iteration_close(g.iterate(300_001, 0, 5), o.iterate(300_001, 5, threads=THREADS))
     g.refine(1.5); o.refine(1.5)
     assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+    g.set_grid(o.get_grid())          # cascade-free: refined edges agree to 1e-12, not bit for bit (libm pow/log)
     assert_events_equal(g.debug_events(0, 3000, 5), o.events(0, 3000, 5), w)
 
     w = W.Workload("toyf", 2, 511, W.TOY_SUM, (), W.FP32_EVAL, 10**5, 1)
@@ -220,6 +221,7 @@ def test_extreme_sizes(V, O):
     assert_iteration_close(g.iterate(200_001, 0, 5), o.iterate(200_001, 5, threads=THREADS))
     g.refine(1.5); o.refine(1.5)
     assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+    g.set_grid(o.get_grid())          # cascade-free: refined edges agree to 1e-12, not bit for bit (libm pow/log)
     assert_events_equal(g.debug_events(0, 3000, 5), o.events(0, 3000, 5), w)
 
     w = W.cfg1()
