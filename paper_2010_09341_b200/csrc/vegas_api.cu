@@ -76,17 +76,19 @@ using AttrFn = cudaError_t (*)(int smem_bytes);
 using OccFn = cudaError_t (*)(int* ctas, int threads, size_t smem);
 
 struct Instance {
-    int integrand_id, dim /* 0 = any */, precision, max_threads;
+    int integrand_id, dim /* 0 = any */, nbins /* 0 = any */, precision;
+    int rs /* log2 histogram replicas, -1 = run-time */, trep /* table replicas */, max_threads;
+    int def_ctas, def_threads;       // default launch shape
     LaunchFn launch;
     DebugFn debug;
     AttrFn set_smem;
     OccFn occupancy;
 };
 
-template <class F, int D, int MAXT, int MINB>
+template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t launch_iterate(const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    iterate_kernel<F, D, MAXT, MINB><<<grid, threads, smem, st>>>(a);
+    iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB><<<grid, threads, smem, st>>>(a);
     return cudaGetLastError();
 }
 template <class F, int D>
@@ -96,43 +98,62 @@ cudaError_t launch_debug(const IterArgs& a, int grid, int threads, cudaStream_t 
     debug_events_kernel<F, D><<<grid, threads, 0, st>>>(a, bins, x, jac, f, wf, pass);
     return cudaGetLastError();
 }
-template <class F, int D, int MAXT, int MINB>
+template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t set_smem_attr(int smem_bytes)
 {
-    return cudaFuncSetAttribute(iterate_kernel<F, D, MAXT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                smem_bytes);
+    return cudaFuncSetAttribute(iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
 }
-template <class F, int D, int MAXT, int MINB>
+template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t query_occupancy(int* ctas, int threads, size_t smem)
 {
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, iterate_kernel<F, D, MAXT, MINB>, threads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB>,
+                                                         threads, smem);
 }
 
-#define VEGAS_INSTANCE(ID, F, D, PREC, MAXT, MINB)                                                       \
-    Instance { ID, D, PREC, MAXT, launch_iterate<F, D, MAXT, MINB>, launch_debug<F, D>,                  \
-               set_smem_attr<F, D, MAXT, MINB>, query_occupancy<F, D, MAXT, MINB> }
+// TUNED: compile-time dim, bin count, replica counts (one per BASELINE.json configuration; the launch
+// shape was chosen by the sweep recorded in DESIGN.md).  GENERIC: everything run-time.
+#define VEGAS_TUNED(ID, F, D, NB, RS, TREP, HB, PREC, MAXT, CTAS, THREADS)                               \
+    Instance { ID, D, NB, PREC, RS, TREP, MAXT, CTAS, THREADS, launch_iterate<F, D, NB, RS, TREP, HB, MAXT, 1>, \
+               launch_debug<F, D>, set_smem_attr<F, D, NB, RS, TREP, HB, MAXT, 1>,                       \
+               query_occupancy<F, D, NB, RS, TREP, HB, MAXT, 1> }
+#define VEGAS_GENERIC(ID, F, D, PREC)                                                                    \
+    Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,          \
+               launch_debug<F, D>, set_smem_attr<F, D, 0, -1, 1, 0, 1024, 1>,                            \
+               query_occupancy<F, D, 0, -1, 1, 0, 1024, 1> }
 
-// Exact-dimension instances for the five configurations and the paper's toy example come first; the
-// D = 0 instances take any dimension up to kMaxDim (run-time loop bounds).
 const Instance kInstances[] = {
-    VEGAS_INSTANCE(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64, 1024, 1),          // configs[0]
-    VEGAS_INSTANCE(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64, 1024, 1),    // configs[1], [2]
-    VEGAS_INSTANCE(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL, 1024, 1),   // configs[3]
-    VEGAS_INSTANCE(VEGAS_LO_2TO2, Lo2to2, 3, VEGAS_FP64, 1024, 1),              // configs[4]
-    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<double>, 10, VEGAS_FP64, 1024, 1),
-    VEGAS_INSTANCE(VEGAS_GAUSS_SYM, GaussSym, 0, VEGAS_FP64, 1024, 1),
-    VEGAS_INSTANCE(VEGAS_GAUSS_DOUBLE, GaussDouble, 0, VEGAS_FP64, 1024, 1),
-    VEGAS_INSTANCE(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 0, VEGAS_FP32_EVAL, 1024, 1),
-    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<double>, 0, VEGAS_FP64, 1024, 1),
-    VEGAS_INSTANCE(VEGAS_TOY_SUM, ToySum<float>, 0, VEGAS_FP32_EVAL, 1024, 1),
+    VEGAS_TUNED(VEGAS_GAUSS_SYM, GaussSym, 4, 50, 5, 8, 4, VEGAS_FP64, 1024, 1, 1024),            // configs[0]
+    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, 50, 5, 8, 8, VEGAS_FP64, 1024, 1, 1024),      // configs[1], [2]
+    VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 4, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
+    VEGAS_TUNED(VEGAS_LO_2TO2, Lo2to2, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),                // configs[4]
+    VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL),
+    VEGAS_GENERIC(VEGAS_LO_2TO2, Lo2to2, 3, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_TOY_SUM, ToySum<double>, 10, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 0, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 0, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 0, VEGAS_FP32_EVAL),
+    VEGAS_GENERIC(VEGAS_TOY_SUM, ToySum<double>, 0, VEGAS_FP64),
+    VEGAS_GENERIC(VEGAS_TOY_SUM, ToySum<float>, 0, VEGAS_FP32_EVAL),
 };
 
-const Instance* find_instance(int id, int dim, int precision)
+// The tuned instance for exactly (id, dim, nbins, precision), or NULL.
+const Instance* find_tuned(int id, int dim, int nbins, int precision)
 {
     for (const Instance& in : kInstances)
-        if (in.integrand_id == id && in.precision == precision && in.dim == dim) return &in;
+        if (in.rs >= 0 && in.integrand_id == id && in.precision == precision && in.dim == dim && in.nbins == nbins) return &in;
+    return nullptr;
+}
+
+// The run-time-shaped instance: exact dimension first, then any dimension.
+const Instance* find_generic(int id, int dim, int precision)
+{
     for (const Instance& in : kInstances)
-        if (in.integrand_id == id && in.precision == precision && in.dim == 0) return &in;
+        if (in.rs < 0 && in.integrand_id == id && in.precision == precision && in.dim == dim) return &in;
+    for (const Instance& in : kInstances)
+        if (in.rs < 0 && in.integrand_id == id && in.precision == precision && in.dim == 0) return &in;
     return nullptr;
 }
 
@@ -152,7 +173,9 @@ int expected_params(int id, int dim)
 
 struct vegas_ctx {
     int dim, nbins, integrand_id, precision;
-    const Instance* inst;
+    const Instance* inst;            // the instance in use (tuned or generic, chosen by apply_shape)
+    const Instance* tuned;           // may be NULL
+    const Instance* generic;
     cudaStream_t stream;
     unsigned char* ws;
     Layout L;
@@ -214,38 +237,46 @@ int setup_integrand(vegas_ctx* c, const double* p)
     }
 }
 
-size_t iterate_smem_bytes(const vegas_ctx* c, int rshift, int threads)
+size_t iterate_smem_bytes(const vegas_ctx* c, const Instance* in, int rshift, int threads)
 {
     const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
     const size_t cell_bytes = (c->precision == VEGAS_FP64) ? 16 : 8;
-    return align_up(cells * (size_t(1) << rshift) * 8, 16) + align_up(cells * cell_bytes, 16) + static_cast<size_t>((threads + 31) / 32) * 5 * 8;
+    return align_up(cells * (size_t(1) << rshift) * 8, 16) + align_up(cells * in->trep * cell_bytes, 16) +
+           static_cast<size_t>((threads + 31) / 32) * 5 * 8;
 }
 
 // Choose R = 2^rshift: the largest power of two <= 32 such that `ctas` CTAs fit in the SM's shared memory.
-int pick_rshift(const vegas_ctx* c, int ctas, int threads)
+int pick_rshift(const vegas_ctx* c, const Instance* in, int ctas, int threads)
 {
     const size_t per_sm = 228u * 1024u;
     for (int rs = 5; rs >= 0; --rs) {
-        const size_t need = iterate_smem_bytes(c, rs, threads) + 1024;   // 1 KB reserved per CTA
+        const size_t need = iterate_smem_bytes(c, in, rs, threads) + 1024;   // 1 KB reserved per CTA
         if (need * ctas <= per_sm && need - 1024 <= static_cast<size_t>(c->smem_optin)) return rs;
     }
     return -1;
 }
 
+// ctas/threads <= 0: the instance's default.  rshift < 0: the tuned instance's fixed R if it can be used,
+// else the largest R that fits.  A shape the tuned instance cannot take (another R) runs on the generic one.
 int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
 {
-    if (threads < 32 || threads > c->inst->max_threads || (threads & 31)) return fail(VEGAS_EINVAL, "threads_per_cta %d not in 32..%d (multiple of 32)", threads, c->inst->max_threads);
+    const Instance* in = (c->tuned && (rshift < 0 || rshift == c->tuned->rs)) ? c->tuned : c->generic;
+    if (ctas <= 0) ctas = in->def_ctas;
+    if (threads <= 0) threads = in->def_threads;
+    if (threads < 32 || threads > in->max_threads || (threads & 31)) return fail(VEGAS_EINVAL, "threads_per_cta %d not in 32..%d (multiple of 32)", threads, in->max_threads);
     if (ctas < 1 || ctas > 16) return fail(VEGAS_EINVAL, "ctas_per_sm %d not in 1..16", ctas);
-    if (rshift < 0) rshift = pick_rshift(c, ctas, threads);
+    if (in->rs >= 0) rshift = in->rs;
+    else if (rshift < 0) rshift = pick_rshift(c, in, ctas, threads);
     if (rshift < 0 || rshift > 5) return fail(VEGAS_EINVAL, "histogram of %d x %d cells does not fit in shared memory with %d CTAs/SM", c->dim, c->nbins, ctas);
-    const size_t smem = iterate_smem_bytes(c, rshift, threads);
+    const size_t smem = iterate_smem_bytes(c, in, rshift, threads);
     if (smem > static_cast<size_t>(c->smem_optin)) return fail(VEGAS_EINVAL, "needs %zu bytes of shared memory per CTA, device allows %d", smem, c->smem_optin);
-    CUDA_TRY(c->inst->set_smem(static_cast<int>(smem)));
+    CUDA_TRY(in->set_smem(static_cast<int>(smem)));
     int occ = 0;
-    CUDA_TRY(c->inst->occupancy(&occ, threads, smem));
+    CUDA_TRY(in->occupancy(&occ, threads, smem));
     if (occ < 1) return fail(VEGAS_EINVAL, "launch shape (%d threads, %zu B smem) cannot run", threads, smem);
     if (occ < ctas) ctas = occ;
     if (ctas * c->sm_count > kMaxSlots) ctas = kMaxSlots / c->sm_count;
+    c->inst = in;
     c->ctas_per_sm = ctas; c->threads = threads; c->rshift = rshift; c->smem_bytes = smem;
     return VEGAS_OK;
 }
@@ -306,7 +337,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     const int need = expected_params(integrand_id, dim);
     if (need < 0) return fail(VEGAS_EUNSUPPORTED, "integrand_id %d unknown", integrand_id);
     if (n_params != need || (need > 0 && !params)) return fail(VEGAS_EINVAL, "integrand %d with dim %d takes %d params, got %d", integrand_id, dim, need, n_params);
-    const Instance* inst = find_instance(integrand_id, dim, precision);
+    const Instance* tuned = find_tuned(integrand_id, dim, nbins, precision);
+    const Instance* inst = find_generic(integrand_id, dim, precision);
     if (!inst) return fail(VEGAS_EUNSUPPORTED, "no compiled kernel for integrand %d, dim %d, precision %d", integrand_id, dim, precision);
     if (!dev_workspace) return fail(VEGAS_EINVAL, "dev_workspace is NULL");
     if (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) return fail(VEGAS_EINVAL, "dev_workspace must be 256-byte aligned");
@@ -321,7 +353,7 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     vegas_ctx* c = new (std::nothrow) vegas_ctx();
     if (!c) return fail(VEGAS_ENOMEM, "host allocation failed");
     c->dim = dim; c->nbins = nbins; c->integrand_id = integrand_id; c->precision = precision;
-    c->inst = inst;
+    c->inst = inst; c->tuned = tuned; c->generic = inst;
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->ws = static_cast<unsigned char*>(dev_workspace);
     c->L = L;
@@ -346,7 +378,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
         cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
         cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess)
         return cleanup(fail(VEGAS_ECUDA, "pinned host buffer / event creation failed: %s", cudaGetErrorString(cudaGetLastError())));
-    rc = apply_shape(c, 2, 512, -1);
+    rc = apply_shape(c, 0, 0, -1);
+    if (rc != VEGAS_OK && c->tuned) { c->tuned = nullptr; rc = apply_shape(c, 0, 0, -1); }
     if (rc != VEGAS_OK) rc = apply_shape(c, 1, 512, -1);
     if (rc != VEGAS_OK) return cleanup(rc);
     if (cudaMemsetAsync(c->ws, 0, L.total, c->stream) != cudaSuccess) return cleanup(fail(VEGAS_ECUDA, "workspace memset failed"));
@@ -370,7 +403,7 @@ void vegas_destroy(vegas_ctx* c)
 int vegas_set_launch_shape(vegas_ctx* c, int ctas_per_sm, int threads_per_cta)
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
-    return apply_shape(c, ctas_per_sm > 0 ? ctas_per_sm : 2, threads_per_cta > 0 ? threads_per_cta : 512, -1);
+    return apply_shape(c, ctas_per_sm, threads_per_cta, -1);
 }
 
 int vegas_set_hist_replicas(vegas_ctx* c, int replicas)

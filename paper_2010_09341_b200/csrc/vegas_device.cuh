@@ -106,6 +106,7 @@ __device__ __forceinline__ void bin_frac32(uint32_t w, uint32_t N, int& i, float
 struct GaussSym {            // I0, BASELINE.json configs[0]
     using real = double;
     static constexpr int kId = 0;
+    static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     double s;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { s = 0.0; }
     __device__ __forceinline__ void coord(int, double x, const IntegrandConsts& c)
@@ -123,6 +124,7 @@ struct GaussSym {            // I0, BASELINE.json configs[0]
 struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
     using real = double;
     static constexpr int kId = 1;
+    static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     double s1, s2;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { s1 = 0.0; s2 = 0.0; }
     __device__ __forceinline__ void coord(int, double x, const IntegrandConsts& c)
@@ -169,6 +171,7 @@ __device__ __forceinline__ float cos_f32(float a)
 struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event arithmetic
     using real = float;
     static constexpr int kId = 2;
+    static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     float arg, Q;
     __device__ __forceinline__ void begin(const IntegrandConsts& c) { arg = c.zphi; Q = 1.0f; }
     __device__ __forceinline__ void coord(int k, float x, const IntegrandConsts& c)
@@ -188,6 +191,7 @@ struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event ari
 struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, v3)
     using real = double;
     static constexpr int kId = 3;
+    static constexpr bool kHasCut = true;   // true: f = 0 for events the integrand's cuts reject
     double v[3];
     __device__ __forceinline__ void begin(const IntegrandConsts&) {}
     __device__ __forceinline__ void coord(int k, double x, const IntegrandConsts&)
@@ -225,6 +229,7 @@ template <typename Real>
 struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1)
     using real = Real;
     static constexpr int kId = 4;
+    static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     Real f;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { f = Real(0); }
     __device__ __forceinline__ void coord(int, Real x, const IntegrandConsts&)

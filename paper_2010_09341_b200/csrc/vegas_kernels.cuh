@@ -58,10 +58,17 @@ __device__ __forceinline__ void comp_warp_reduce(Comp& c)
 // the histogram, both in shared memory.  HBM: one table read per CTA at entry, one d*N flush per CTA
 // at exit (global fp64 reductions), four doubles per CTA for the scalar sums.
 //
-// Shared memory:  hist[d*N][R] fp64 (R = 2^rshift lane-indexed replicas: lane l updates replica l%R, so
-//                 with R = 32 no two lanes of a warp ever touch the same word and the compare-and-swap
-//                 that fp64 shared atomics compile to on sm_100a succeeds first try unless another
-//                 warp got in between) | table[d*N] real2 | per-warp partial sums.
+// Shared memory:  hist[d*N][R] fp64 | table[d*N][TREP] real2 | per-warp partial sums.
+//   hist : R = 2^rshift lane-indexed replicas; lane l updates replica l%R, so with R = 32 no two lanes of a
+//          warp ever touch the same word and the compare-and-swap that an fp64 shared-memory add is on
+//          sm_100a (LDS, DADD, ATOMS.CAST) succeeds first try unless another warp got in between.
+//   table: TREP lane-indexed copies of every 16-byte (fp64) / 8-byte (fp32) cell, lane l reads copy
+//          l%TREP.  A 16-byte shared load is served one quarter-warp (8 lanes) per wavefront; with TREP = 8
+//          the 8 lanes hit 8 different 4-bank groups whatever their bins are, so the random-bin lookup
+//          costs the minimum 4 wavefronts instead of the ~9.6 measured without replication (profiles/r01a).
+// Template parameters: D, NB compile-time dimension / bin count (0 = run-time a.dim / a.nbins); RS
+// compile-time log2 R (-1 = run-time a.rshift); TREP; HB = number of histogram updates whose
+// compare-and-swap sequences are issued together (0 = one atomicAdd spin loop per update).
 // Grid: a multiple of the SM count; the events of the launch are dealt round-robin to threads
 // (idx = blockIdx*blockDim + tid, stride gridDim*blockDim), so the Philox counter of a thread's next
 // event is its previous one plus a constant.
@@ -78,7 +85,52 @@ struct BinPack {   // d bin indices, 16 bits each, kept in registers (all indice
     __device__ __forceinline__ int get(int k) const { return static_cast<int>((w[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu); }
 };
 
-template <class F, int D, int MAXT, int MINB>
+__device__ __forceinline__ unsigned long long lds_u64(const double* p)
+{
+    unsigned long long v;
+    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(p))) : "memory");
+    return v;
+}
+
+// H[k][bin_k] += q for the dims [k0, k0 + HB): all loads, then all adds, then all compare-and-swaps, so
+// the HB dependent chains (LDS -> DADD -> ATOMS.CAS) overlap; a lost race (another warp updated the
+// same replica word in between -- rare with lane-indexed replicas) is redone with the spin loop.
+template <int D, int HB>
+__device__ __forceinline__ void hist_update_batch(double* hlane, int k0, int d, int N, int rs, const BinPack<D>& bp,
+                                                  double q)
+{
+    double* p[HB];
+    unsigned long long o[HB], n[HB];
+#pragma unroll
+    for (int j = 0; j < HB; ++j) {
+        const int k = k0 + j;
+        if (k < d) {
+            p[j] = hlane + (static_cast<size_t>(k * N + bp.get(k)) << rs);
+            o[j] = lds_u64(p[j]);
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < HB; ++j)
+        if (k0 + j < d) n[j] = static_cast<unsigned long long>(__double_as_longlong(__dadd_rn(__longlong_as_double(static_cast<long long>(o[j])), q)));
+    bool lost = false;
+    bool lostj[HB];
+#pragma unroll
+    for (int j = 0; j < HB; ++j) {
+        lostj[j] = false;
+        if (k0 + j < d) {
+            const unsigned long long r = atomicCAS(reinterpret_cast<unsigned long long*>(p[j]), o[j], n[j]);
+            lostj[j] = (r != o[j]);
+            lost |= lostj[j];
+        }
+    }
+    if (lost) {
+#pragma unroll
+        for (int j = 0; j < HB; ++j)
+            if (lostj[j]) atomicAdd(p[j], q);
+    }
+}
+
+template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
 {
     using real = typename F::real;
@@ -86,25 +138,26 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int d = D ? D : a.dim;
-    const int N = a.nbins;
+    const int N = NB ? NB : a.nbins;
+    const int rs = (RS >= 0) ? RS : a.rshift;
     const int cells = d * N;
-    const int R = 1 << a.rshift;
+    const int R = 1 << rs;
     const size_t hist_bytes = (static_cast<size_t>(cells) * R * sizeof(double) + 15) & ~size_t(15);
+    const size_t tab_bytes = (static_cast<size_t>(cells) * TREP * sizeof(real2) + 15) & ~size_t(15);
     double* sh_hist = reinterpret_cast<double*>(smem_raw);
     real2* sh_tab = reinterpret_cast<real2*>(smem_raw + hist_bytes);
-    double* sh_part = reinterpret_cast<double*>(smem_raw + hist_bytes +
-                                                ((static_cast<size_t>(cells) * sizeof(real2) + 15) & ~size_t(15)));
+    double* sh_part = reinterpret_cast<double*>(smem_raw + hist_bytes + tab_bytes);
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
     for (int i = tid; i < cells * R; i += blockDim.x) sh_hist[i] = 0.0;
     {
         const real2* gt = static_cast<const real2*>(a.table);
-        for (int i = tid; i < cells; i += blockDim.x) sh_tab[i] = gt[i];
+        for (int i = tid; i < cells * TREP; i += blockDim.x) sh_tab[i] = gt[i / TREP];
     }
     __syncthreads();
 
-    const int rep = lane & (R - 1);
+    double* hlane = sh_hist + (lane & (R - 1));
     Comp s1{0.0, 0.0}, s2{0.0, 0.0};
     unsigned int np = 0;
 
@@ -114,17 +167,26 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
         bp.clear();
         real J, f;
         bool pass;
-        const double wf = process_event<F, D, 0, 1>(
-            a, a.e_lo_first + idx, sh_tab, 0, [&](int k, int i, real) { bp.set(k, i); }, J, f, pass);
+        const double wf = process_event<F, D, NB, TREP>(
+            a, a.e_lo_first + idx, sh_tab, lane & (TREP - 1), [&](int k, int i, real) { bp.set(k, i); }, J, f, pass);
         const double q = __dmul_rn(wf, wf);                       // S4
         kahan_add(s1, wf);                                        // S5
         kahan_add(s2, q);
         np += pass ? 1u : 0u;
-        if (q != 0.0) {                                           // adding 0 is the identity (reading R8)
+        // adding 0 is the identity (reading R8): events cut away by the integrand skip the histogram
+        if (!F::kHasCut || q != 0.0) {
+            if constexpr (HB > 0) {
 #pragma unroll
-            for (int k = 0; k < (D ? D : kMaxDim); ++k) {
-                if (!D && k >= d) break;
-                atomicAdd(&sh_hist[((k * N + bp.get(k)) << a.rshift) + rep], q);
+                for (int k0 = 0; k0 < (D ? D : kMaxDim); k0 += HB) {
+                    if (!D && k0 >= d) break;
+                    hist_update_batch<D, HB>(hlane, k0, d, N, rs, bp, q);
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < (D ? D : kMaxDim); ++k) {
+                    if (!D && k >= d) break;
+                    atomicAdd(hlane + (static_cast<size_t>(k * N + bp.get(k)) << rs), q);
+                }
             }
         }
     }
@@ -156,9 +218,9 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 
     // ---- histogram flush: fixed-order sum over the replicas, one global reduction per touched cell ----
     for (int c = tid; c < cells; c += blockDim.x) {
-        const double* p = sh_hist + (static_cast<size_t>(c) << a.rshift);
-        double v = p[0];
-        for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[r]);
+        const double* p = sh_hist + (static_cast<size_t>(c) << rs);
+        double v = p[c & (R - 1)];                              // rotated start: conflict-free reads
+        for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[(r + c) & (R - 1)]);
         if (v != 0.0) atomicAdd(a.hist + c, v);
     }
 }
