@@ -144,6 +144,20 @@ const char* vegas_last_error(void);
  * context runs on. */
 int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
 
+/* Measured instruction throughput (thread-instructions per second over the whole GPU, current clocks) of
+ * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports
+ * (BASELINE.json north_star: "fraction of the FP pipe roofline").  Each call runs a
+ * few milliseconds of 8 independent dependency chains per thread at full occupancy on `cuda_stream`
+ * (NULL = default stream) and synchronises.  No context needed.
+ *   VEGAS_PIPE_DFMA            fp64 fused multiply-add   (peak FLOP/s = 2 x rate)
+ *   VEGAS_PIPE_FFMA            fp32 fused multiply-add
+ *   VEGAS_PIPE_IMAD_WIDE       32x32->64 integer multiply (two per Philox round)
+ *   VEGAS_PIPE_LOP3            three-input logic op (two per Philox round)
+ *   VEGAS_PIPE_SHARED_F64_ADD  fp64 atomicAdd on shared memory, lane-indexed replicas, random cells
+ * Errors: VEGAS_EINVAL (unknown pipe, NULL out), VEGAS_ECUDA. */
+enum { VEGAS_PIPE_DFMA = 0, VEGAS_PIPE_FFMA = 1, VEGAS_PIPE_IMAD_WIDE = 2, VEGAS_PIPE_LOP3 = 3, VEGAS_PIPE_SHARED_F64_ADD = 4 };
+int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr_per_s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -15,7 +15,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libvegas_b200.so")
-SOURCES = [os.path.join(CSRC, "vegas_api.cu")]
+SOURCES = [os.path.join(CSRC, "vegas_api.cu"), os.path.join(CSRC, "pipe_bench.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "vegas_kernels.cuh"), os.path.join(CSRC, "vegas_device.cuh"),
                   os.path.join(INCLUDE, "vegas_b200.h")]
 

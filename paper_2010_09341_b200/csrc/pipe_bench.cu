@@ -1,0 +1,117 @@
+// pipe_bench.cu -- vegas_pipe_rate(): instruction-throughput microbenchmarks of the SM pipes the Vegas hot
+// path runs on.  They are the measured denominators of the roofline bench.py reports:
+// the path moves no HBM bytes per event and is no tensor-core contraction, so its bound is the issue rate of
+// the FP64 pipe (DFMA/DADD/DMUL), of the FP32 pipes (FFMA), of the wide integer multiplier Philox needs
+// (IMAD.WIDE.U32), of the logic pipe (LOP3) and of the shared-memory compare-and-swap an fp64 histogram
+// update is on sm_100a.  Measured in the same process, right before the timed region, because the SM clock
+// under load is not the nominal one.
+#include <cstdint>
+#include <cuda_runtime.h>
+
+#include "../../include/vegas_b200.h"
+
+namespace {
+
+constexpr int kChains = 8;    // independent dependency chains per thread
+constexpr int kUnroll = 16;   // operations per chain per loop trip
+
+template <int KIND>
+__global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long long* out, uint32_t seed)
+{
+    extern __shared__ double sh[];                     // KIND 4: [32 cells][32 lanes]
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    double d[kChains];
+    float f[kChains];
+    unsigned long long w[kChains];
+    uint32_t u[kChains], v[kChains];
+#pragma unroll
+    for (int c = 0; c < kChains; ++c) {
+        d[c] = 1.0 + 1e-9 * (t + c);
+        f[c] = 1.0f + 1e-6f * (t + c);
+        w[c] = static_cast<unsigned long long>(t * 7u + c) * 0x9E3779B97F4A7C15ull + seed;
+        u[c] = t * 31u + c + seed;
+        v[c] = t * 17u + c * 3u + seed;
+    }
+    if (KIND == 4) {
+        for (int i = threadIdx.x; i < 32 * 32; i += blockDim.x) sh[i] = 0.0;
+        __syncthreads();
+    }
+    const double da = 1.0000001, db = 1e-9;
+    const float fa = 1.0001f, fb = 1e-6f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int j = 0; j < kUnroll; ++j) {
+#pragma unroll
+            for (int c = 0; c < kChains; ++c) {
+                if (KIND == 0) d[c] = __fma_rn(d[c], da, db);
+                if (KIND == 1) f[c] = __fmaf_rn(f[c], fa, fb);
+                if (KIND == 2) asm volatile("mad.wide.u32 %0, %1, %2, 0;" : "=l"(w[c]) : "r"(static_cast<uint32_t>(w[c] >> 32)), "r"(0xD2511F53u));
+                if (KIND == 3) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[c]) : "r"(v[c]), "r"(seed));
+                if (KIND == 4) {
+                    // one fp64 histogram update: lane-indexed replica (conflict-free within the warp), pseudo-random cell
+                    u[c] = u[c] * 1664525u + 1013904223u;
+                    atomicAdd(&sh[((u[c] >> 27) << 5) + (threadIdx.x & 31)], db);
+                }
+            }
+        }
+    }
+    unsigned long long acc = 0;
+#pragma unroll
+    for (int c = 0; c < kChains; ++c)
+        acc += static_cast<unsigned long long>(__double_as_longlong(d[c])) + __float_as_uint(f[c]) + w[c] + u[c] + v[c];
+    if (acc == 0x1234567ull) out[t] = acc;             // never true in practice: keeps the chains alive
+}
+
+template <int KIND>
+cudaError_t time_kind(int sms, int iters, unsigned long long* out, cudaStream_t st, double* rate)
+{
+    const int blocks = sms * 2, threads = 1024;
+    const size_t smem = (KIND == 4) ? 32 * 32 * sizeof(double) : 0;
+    cudaEvent_t e0, e1;
+    cudaError_t e = cudaEventCreate(&e0);
+    if (e != cudaSuccess) return e;
+    e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    float best = 0.f;
+    for (int r = 0; r < 3 && e == cudaSuccess; ++r) {  // first pass warms up; best of the next two
+        cudaEventRecord(e0, st);
+        pipe_kernel<KIND><<<blocks, threads, smem, st>>>(iters, out, 12345u + r);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && (best == 0.f || ms < best)) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess) return e;
+    const double ops = static_cast<double>(iters) * kUnroll * kChains * blocks * threads;
+    *rate = ops / (best * 1e-3);
+    return cudaSuccess;
+}
+
+}  // namespace
+
+extern "C" int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr_per_s)
+{
+    if (!thread_instr_per_s) return VEGAS_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+        (void)cudaGetLastError();
+        return VEGAS_ECUDA;
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    unsigned long long* out = nullptr;
+    if (cudaMalloc(reinterpret_cast<void**>(&out), static_cast<size_t>(sms) * 2 * 1024 * 8) != cudaSuccess) return VEGAS_ECUDA;
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (pipe) {
+        case VEGAS_PIPE_DFMA: e = time_kind<0>(sms, 1000, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_FFMA: e = time_kind<1>(sms, 2000, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_IMAD_WIDE: e = time_kind<2>(sms, 500, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_LOP3: e = time_kind<3>(sms, 1000, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_SHARED_F64_ADD: e = time_kind<4>(sms, 100, out, st, thread_instr_per_s); break;
+        default: cudaFree(out); return VEGAS_EINVAL;
+    }
+    cudaFree(out);
+    return e == cudaSuccess ? VEGAS_OK : VEGAS_ECUDA;
+}

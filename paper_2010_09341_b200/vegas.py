@@ -40,6 +40,7 @@ SIGNATURES = {
     "vegas_set_hist_replicas": (C.c_int, [_vp, C.c_int]),
     "vegas_get_launch_shape": (C.c_int, [_vp, _ip, _ip, _ip, _szp]),
     "vegas_device_info": (C.c_int, [_vp, _ip, _ip]),
+    "vegas_pipe_rate": (C.c_int, [C.c_int, _vp, _dp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
 }
@@ -199,6 +200,17 @@ class Vegas:
         a, b = C.c_int(), C.c_int()
         _chk(lib().vegas_device_info(self._h, C.byref(a), C.byref(b)), "vegas_device_info")
         return dict(sm_count=a.value, sm_clock_khz=b.value)
+
+
+PIPE_DFMA, PIPE_FFMA, PIPE_IMAD_WIDE, PIPE_LOP3, PIPE_SHARED_F64_ADD = 0, 1, 2, 3, 4
+
+
+def pipe_rate(pipe, stream=None):
+    """Measured thread-instructions/s of one SM pipe (vegas_pipe_rate): the roofline denominators."""
+    v = C.c_double()
+    _chk(lib().vegas_pipe_rate(int(pipe), _vp(stream.cuda_stream) if stream is not None else None, C.byref(v)),
+         "vegas_pipe_rate")
+    return v.value
 
 
 def from_workload(w, **kw):
