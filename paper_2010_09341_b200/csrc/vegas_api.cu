@@ -79,6 +79,7 @@ struct Instance {
     int integrand_id, dim /* 0 = any */, nbins /* 0 = any */, precision;
     int rs /* log2 histogram replicas, -1 = run-time */, trep /* table replicas */, max_threads;
     int def_ctas, def_threads;       // default launch shape
+    int queue_entry_bytes;           // per-entry bytes of the per-warp compaction queue (0: integrand has no cut)
     LaunchFn launch;
     DebugFn debug;
     AttrFn set_smem;
@@ -111,14 +112,20 @@ cudaError_t query_occupancy(int* ctas, int threads, size_t smem)
                                                          threads, smem);
 }
 
+template <class F, int D>
+constexpr int queue_entry_bytes()
+{
+    return F::kHasCut ? static_cast<int>(sizeof(F) + 8 + ((sizeof(BinPack<D>) / 4 + 1) / 2) * 8) : 0;
+}
+
 // TUNED: compile-time dim, bin count, replica counts (one per BASELINE.json configuration; the launch
 // shape was chosen by the sweep recorded in DESIGN.md).  GENERIC: everything run-time.
 #define VEGAS_TUNED(ID, F, D, NB, RS, TREP, HB, PREC, MAXT, CTAS, THREADS)                               \
-    Instance { ID, D, NB, PREC, RS, TREP, MAXT, CTAS, THREADS, launch_iterate<F, D, NB, RS, TREP, HB, MAXT, 1>, \
+    Instance { ID, D, NB, PREC, RS, TREP, MAXT, CTAS, THREADS, queue_entry_bytes<F, D>(), launch_iterate<F, D, NB, RS, TREP, HB, MAXT, 1>, \
                launch_debug<F, D>, set_smem_attr<F, D, NB, RS, TREP, HB, MAXT, 1>,                       \
                query_occupancy<F, D, NB, RS, TREP, HB, MAXT, 1> }
 #define VEGAS_GENERIC(ID, F, D, PREC)                                                                    \
-    Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,          \
+    Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, queue_entry_bytes<F, D>(), launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,          \
                launch_debug<F, D>, set_smem_attr<F, D, 0, -1, 1, 0, 1024, 1>,                            \
                query_occupancy<F, D, 0, -1, 1, 0, 1024, 1> }
 
@@ -242,7 +249,7 @@ size_t iterate_smem_bytes(const vegas_ctx* c, const Instance* in, int rshift, in
     const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
     const size_t cell_bytes = (c->precision == VEGAS_FP64) ? 16 : 8;
     return align_up(cells * (size_t(1) << rshift) * 8, 16) + align_up(cells * in->trep * cell_bytes, 16) +
-           static_cast<size_t>((threads + 31) / 32) * 5 * 8;
+           static_cast<size_t>((threads + 31) / 32) * (5 * 8 + static_cast<size_t>(in->queue_entry_bytes) * kQueueCap);
 }
 
 // Choose R = 2^rshift: the largest power of two <= 32 such that `ctas` CTAs fit in the SM's shared memory.

@@ -114,9 +114,9 @@ struct GaussSym {            // I0, BASELINE.json configs[0]
         const double dx = __dsub_rn(x, c.gmu0);
         s = __fma_rn(dx, dx, s);
     }
-    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
     {
-        pass = true;
         return __dmul_rn(c.gC, exp(-__dmul_rn(s, c.ga2)));
     }
 };
@@ -133,9 +133,9 @@ struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
         s1 = __fma_rn(d1, d1, s1);
         s2 = __fma_rn(d2, d2, s2);
     }
-    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
     {
-        pass = true;
         const double e1 = exp(-__dmul_rn(s1, c.ga2));
         const double e2 = exp(-__dmul_rn(s2, c.ga2));
         return __dmul_rn(__dmul_rn(0.5, c.gC), __dadd_rn(e1, e2));
@@ -181,9 +181,9 @@ struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event ari
         const float pk = __fmaf_rn(dx, dx, c.zw[k]);
         Q = __fmul_rn(Q, pk);
     }
-    __device__ __forceinline__ float end(const IntegrandConsts&, int, bool& pass)
+    __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
+    __device__ __forceinline__ float end(const IntegrandConsts&, int) const
     {
-        pass = true;
         return __fdiv_rn(cos_f32(arg), Q);
     }
 };
@@ -198,13 +198,18 @@ struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, 
     {
         if (k == 0) v[0] = x; else if (k == 1) v[1] = x; else v[2] = x;
     }
-    __device__ __forceinline__ double end(const IntegrandConsts& c, int, bool& pass)
+    // the cuts, on exactly rounded quantities so that the selection is bit-reproducible (reading R15)
+    __device__ __forceinline__ bool precheck(const IntegrandConsts& c) const
+    {
+        const double cth = __fma_rn(2.0, v[2], -1.0);
+        return (__dadd_rn(v[0], v[1]) < 1.0) && (fabs(cth) < c.hcut);
+    }
+    // value for an event that passed precheck()
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
     {
         const double v1 = v[0], v2 = v[1], v3 = v[2];
         const double L = c.hL, s = c.hs;
         const double cth = __fma_rn(2.0, v3, -1.0);
-        pass = (__dadd_rn(v1, v2) < 1.0) && (fabs(cth) < c.hcut);   // cuts on exactly rounded quantities
-        if (!pass) return 0.0;
         const double x1 = exp(__dmul_rn(v1, L));
         const double x2 = exp(__dmul_rn(v2, L));
         const double x12 = __dmul_rn(x1, x2);
@@ -236,7 +241,8 @@ struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1
     {
         if constexpr (sizeof(Real) == 8) f = __dadd_rn(f, x); else f = __fadd_rn(f, x);
     }
-    __device__ __forceinline__ Real end(const IntegrandConsts&, int, bool& pass) { pass = true; return f; }
+    __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
+    __device__ __forceinline__ Real end(const IntegrandConsts&, int) const { return f; }
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -245,22 +251,16 @@ struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1
 // tab[(k*N + i) * TSTRIDE + toff] (TSTRIDE/toff implement lane-replicated bank-conflict-free copies).
 // bins[] receives the d bin indices.  Returns wf = (double)J * (double)f.
 // ------------------------------------------------------------------------------------------------
-template <class F, int D, int NB>
-struct EventOut {
-    double wf;
-    bool pass;
-};
-
+// event_front: S1 + S2 + the per-coordinate part of S3.  Leaves the integrand's accumulated state in
+// `integrand` and returns J.
 template <class F, int D, int NB, int TSTRIDE, class BinSink>
-__device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
-                                                BinSink&& sink, typename F::real& J_out,
-                                                typename F::real& f_out, bool& pass)
+__device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
+                                                        BinSink&& sink, F& integrand)
 {
     using real = typename F::real;
     constexpr bool kF64 = (sizeof(real) == 8);
     const int d = D ? D : a.dim;
     const uint32_t N = NB ? static_cast<uint32_t>(NB) : static_cast<uint32_t>(a.nbins);
-    F integrand;
     integrand.begin(a.ic);
     real J = real(1);
     uint32_t r[4] = {0u, 0u, 0u, 0u};
@@ -299,7 +299,20 @@ __device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo
             integrand.coord(k, x, a.ic);
         }
     }
-    const real f = integrand.end(a.ic, d, pass);
+    return J;
+}
+
+// One whole event, S1-S4: returns wf = (double)J * (double)f.
+template <class F, int D, int NB, int TSTRIDE, class BinSink>
+__device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
+                                                BinSink&& sink, typename F::real& J_out,
+                                                typename F::real& f_out, bool& pass)
+{
+    using real = typename F::real;
+    F integrand;
+    const real J = event_front<F, D, NB, TSTRIDE>(a, e_lo, tab_, toff, sink, integrand);
+    pass = integrand.precheck(a.ic);
+    const real f = pass ? integrand.end(a.ic, D ? D : a.dim) : real(0);
     J_out = J;
     f_out = f;
     return __dmul_rn(static_cast<double>(J), static_cast<double>(f));   // S4
