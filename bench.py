@@ -174,6 +174,22 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------
 # the B200 arm
 # ---------------------------------------------------------------------------------------------------
+def max_over_ranks(values, device="cpu"):
+    """Element-wise maximum of a list of floats over all ranks (identity without a process group): the
+    replicas-only multi-GPU timing rule -- every rank reports the slowest rank's time."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(values, dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def aggregate_value(events_per_rank_step, steps, world, ms):
+    """Whole-job throughput of `world` independent replicas: all ranks' events over the slowest rank's time."""
+    return float(events_per_rank_step) * steps * world / (ms * 1e-3)
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -245,14 +261,11 @@ def run_b200(args):
     torch.cuda.synchronize(dev)
     e2e_ms = (time.perf_counter() - t0) * 1e3
 
-    times = torch.tensor([dev_ms, e2e_ms, iter_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(times, op=dist.ReduceOp.MAX)
-    dev_ms, e2e_ms, iter_ms = [float(v) for v in times.tolist()]
+    dev_ms, e2e_ms, iter_ms = max_over_ranks([dev_ms, e2e_ms, iter_ms], dev)
 
     if rank == 0:
         total_events = float(n) * args.steps * world
-        value = total_events / (dev_ms * 1e-3)
+        value = aggregate_value(n, args.steps, world, dev_ms)
         dt = dtype_of(w)
         kern_s = iter_ms * 1e-3 / args.steps          # average duration of one iteration's kernels
         fpe = ALGO_FLOPS[args.workload]
