@@ -39,6 +39,10 @@ UNIT = "events/s"
 ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg4": 232.0, "cfg5": (130.0, 14.0)}
 # FP pipe lanes per SM (B200): 64 fp64, 128 fp32.  Peak = SMs * lanes * 2 FLOP * max SM clock.
 FP_LANES = {"f64": 64, "f32": 128}
+# dram__bytes_read.sum + dram__bytes_write.sum of one 1e8-event iterate_kernel launch, from the ncu --set full
+# captures summarised in profiles/r01c_ncu_full_<cfg>_iterate.md (the algorithmic HBM traffic is ~0: one table
+# read and one d*N flush per CTA)
+NCU_TRAFFIC_BYTES = {"cfg2": 36352, "cfg4": 73216, "cfg5": 44032}
 
 
 def parse_args():
@@ -285,7 +289,8 @@ def run_b200(args):
                     "note": "vegas_iterate + vegas_refine with host result buffers, host wall clock"},
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "iterate_kernel", "kernel_ms": kern_s * 1e3,
+                         "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if n == w.n_events and epl == n else None,
+                         "traffic_unit": "bytes per launch (ncu, profiles/r01c_*)", "kernel": "iterate_kernel", "kernel_ms": kern_s * 1e3,
                          "flops_per_event": fpe,
                          "peak_source": "SMs x %d %s lanes x 2 x max SM clock (B200 unit counts; DESIGN.md section 7)" % (FP_LANES[dt], dt),
                          "peak_measured": peak_measured, "frac_of_measured": achieved / peak_measured,
