@@ -132,7 +132,7 @@ constexpr int queue_entry_bytes()
 const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GAUSS_SYM, GaussSym, 4, 50, 5, 8, 4, VEGAS_FP64, 1024, 1, 1024),            // configs[0]
     VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, 50, 5, 8, 8, VEGAS_FP64, 1024, 1, 1024),      // configs[1], [2]
-    VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 4, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
+    VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 0, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
     VEGAS_TUNED(VEGAS_LO_2TO2, Lo2to2, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),                // configs[4]
     VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64),

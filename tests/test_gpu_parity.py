@@ -303,3 +303,55 @@ def test_estimates_within_4_sigma_of_closed_form(V, golden_dir):
             I, s, _ = g.iterate(10**6, 0, w.seed)
             g.refine(w.alpha)
         assert abs(I - target) <= 4 * s, (name, I, s)
+
+
+# ---------------------------------------------------------------------------------------------------
+# BASELINE.json full sizes, in the launch configuration bench.py times (one launch per iteration, the
+# instance's default shape)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
+def test_full_size_iteration_parity(V, O, name):
+    """1e8 events: iteration 0 on the uniform grid and iteration 1 on the oracle's refined grid
+    (cascade-free), I / sigma rel 1e-12, every histogram cell rel 1e-10, pass count exact, plus sampled events
+    from the far end of the index range compared one by one."""
+    w = small_workloads()[name]
+    assert w.n_events == 10**8
+    g, o = make_pair(V, O, w)
+    for it in range(2):
+        ores = o.iterate(w.n_events, w.seed, threads=THREADS)
+        gres = g.iterate(w.n_events, 0, w.seed)
+        assert g.launch_shape()["ctas_per_sm"] * g.launch_shape()["threads_per_cta"] >= 512
+        assert_iteration_close(gres, ores)
+        if o.npass is not None:
+            assert g.last_npass() == o.npass
+        S2 = g.last_sums()[1]
+        np.testing.assert_allclose(gres[2].sum(axis=1), S2, rtol=1e-12)
+        g.set_iteration(it)
+        o.set_iteration(it)
+        assert_events_equal(g.debug_events(w.n_events - 4096, 4096, seed=w.seed),
+                            o.events(w.n_events - 4096, 4096, w.seed), w)
+        g.set_iteration(it + 1)
+        o.set_iteration(it + 1)
+        o.refine(w.alpha)
+        g.refine(w.alpha)
+        assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+        g.set_grid(o.get_grid())
+
+
+def test_batch_size_study_shape(V):
+    """configs[2] / PAPER.md:L65: throughput suffers when the batch is too small and reaches a plateau.
+    Loose, timing-based: 1e4-event launches are at least 5x slower per event than 1e7-event launches, and
+    1e7 is within 25 % of the single-launch time."""
+    w = W.cfg2(n_events=10**7)
+    g = V.from_workload(w)
+    ms = {}
+    for epl in (10**4, 10**6, 10**7):
+        g.reset()
+        g.iterate(w.n_events, epl, w.seed, want_hist=False)          # warm-up
+        best = 1e30
+        for _ in range(3):
+            g.iterate(w.n_events, epl, w.seed, want_hist=False)
+            best = min(best, g.last_sums()[2])
+        ms[epl] = best
+    assert ms[10**4] > 5 * ms[10**7], ms
+    assert ms[10**6] >= 0.95 * ms[10**7] and ms[10**6] < 2.5 * ms[10**7], ms
