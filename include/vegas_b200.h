@@ -144,6 +144,24 @@ const char* vegas_last_error(void);
  * context runs on. */
 int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
 
+/* run_integration (PAPER.md:L79 `integrator.run_integration(n_iter, log_time=True)`, L88 "every iteration informs
+ * the subsequent run"): n_warmup + n_iter times { vegas_iterate(n_events, events_per_launch, seed);
+ * vegas_refine(alpha) }, then the classic Vegas combination of the last n_iter iterations (the warm-up ones only
+ * adapt the grid; paper silent on the formula, reading R18 in DESIGN.md):
+ *     w_i = 1/sigma_i^2,  mean = sum w_i I_i / sum w_i,  error = 1/sqrt(sum w_i),
+ *     chi2_dof = sum w_i (I_i - mean)^2 / (n_iter - 1)           (0 when n_iter = 1)
+ * Iterations with sigma_i = 0 (or not finite) carry no weight; if none has weight: mean = plain average, error = 0.
+ * iter_integral / iter_error / iter_kernel_ms (each n_warmup + n_iter doubles, host, may be NULL) receive every
+ * iteration's estimate and device time (the `log_time` of the paper's call).  A refine that fails with
+ * VEGAS_EGRID leaves the grid as it was and the run goes on.  The per-iteration work runs in the kernels; the
+ * combination is host arithmetic over n_iter numbers (vegas_combine_iterations, callable on its own, no GPU).
+ * Errors: VEGAS_EINVAL (n_iter < 1, n_warmup < 0, NULL mean/error, iterate's argument errors), VEGAS_ECUDA. */
+int vegas_run_integration(vegas_ctx* ctx, int n_iter, int n_warmup, uint64_t n_events, uint64_t events_per_launch,
+                          uint64_t seed, double alpha, double* mean, double* error, double* chi2_dof,
+                          double* iter_integral, double* iter_error, double* iter_kernel_ms);
+int vegas_combine_iterations(int n, const double* integral, const double* error, double* mean, double* comb_error,
+                             double* chi2_dof);
+
 /* Measured instruction throughput (thread-instructions per second over the whole GPU, current clocks) of
  * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports
  * (BASELINE.json north_star: "fraction of the FP pipe roofline").  Each call runs a

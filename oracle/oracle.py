@@ -75,6 +75,7 @@ def lib():
         L.oracle_refine.argtypes = [vp, C.c_double]
         L.oracle_get_table.argtypes = [vp, dp, dp, dp]
         L.oracle_get_gauss_consts.argtypes = [vp, dp]
+        L.oracle_combine.argtypes = [C.c_int, dp, dp, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -233,3 +234,26 @@ class Oracle:
 
     def refine(self, alpha):
         _chk(lib().oracle_refine(self._h, float(alpha)), "refine")
+
+    def run_integration(self, n_iter, n_events, seed, alpha, n_warmup=0, threads=1):
+        """(n_warmup + n_iter) x (iterate, refine); combination of the last n_iter (oracle_combine).
+        A refine rejected for a non-monotone grid (EGRID) leaves the grid unchanged and the run goes on."""
+        I, s = [], []
+        for _ in range(n_warmup + n_iter):
+            res = self.iterate(n_events, seed, threads=threads)
+            I.append(res[0]); s.append(res[1])
+            try:
+                self.refine(alpha)
+            except OracleError as e:
+                if e.code != EGRID:
+                    raise
+        return (*combine(I[n_warmup:], s[n_warmup:]), np.array(I), np.array(s))
+
+
+def combine(integral, sigma):
+    """oracle_combine: inverse-variance average, its error and chi2/dof."""
+    I = np.ascontiguousarray(integral, dtype=np.float64)
+    s = np.ascontiguousarray(sigma, dtype=np.float64)
+    m, e, c2 = C.c_double(), C.c_double(), C.c_double()
+    _chk(lib().oracle_combine(int(I.size), _dp(I), _dp(s), C.byref(m), C.byref(e), C.byref(c2)), "combine")
+    return m.value, e.value, c2.value

@@ -665,3 +665,42 @@ int oracle_get_gauss_consts(const oracle_ctx *c, double *out)
     out[0] = c->gC; out[1] = c->ga2;
     return ORACLE_OK;
 }
+
+/*
+ * run_integration (the combination formula is paper-silent: DESIGN.md reading R18, the classic
+ * Vegas inverse-variance average of the cited references).
+ *   w_i = 1/sigma_i^2 ; mean = (sum_i w_i I_i)/(sum_i w_i) ; error = 1/sqrt(sum_i w_i) ;
+ *   chi2/dof = (sum_i w_i (I_i - mean)^2)/(n - 1)    (0 for n = 1)
+ * Iterations whose sigma is zero or not finite carry no weight; if none does: plain average, error 0.
+ */
+int oracle_combine(int n, const double *I, const double *sigma, double *mean, double *err, double *chi2_dof)
+{
+    if (n < 1 || !I || !sigma || !mean || !err) return ORACLE_EINVAL;
+    long double sum_w = 0.0L, sum_wi = 0.0L, sum_plain = 0.0L;
+    int used = 0;
+    for (int i = 0; i < n; ++i) {
+        sum_plain += (long double)I[i];
+        if (sigma[i] > 0.0 && isfinite(sigma[i]) && isfinite(I[i])) {
+            long double w = 1.0L / ((long double)sigma[i] * (long double)sigma[i]);
+            sum_w += w;
+            sum_wi += w * (long double)I[i];
+            ++used;
+        }
+    }
+    if (used == 0) {
+        *mean = (double)(sum_plain / n);
+        *err = 0.0;
+        if (chi2_dof) *chi2_dof = 0.0;
+        return ORACLE_OK;
+    }
+    long double m = sum_wi / sum_w, chi2 = 0.0L;
+    for (int i = 0; i < n; ++i)
+        if (sigma[i] > 0.0 && isfinite(sigma[i]) && isfinite(I[i])) {
+            long double w = 1.0L / ((long double)sigma[i] * (long double)sigma[i]);
+            chi2 += w * ((long double)I[i] - m) * ((long double)I[i] - m);
+        }
+    *mean = (double)m;
+    *err = (double)(1.0L / sqrtl(sum_w));
+    if (chi2_dof) *chi2_dof = (n > 1) ? (double)(chi2 / (n - 1)) : 0.0;
+    return ORACLE_OK;
+}

@@ -562,6 +562,66 @@ int vegas_refine(vegas_ctx* c, double alpha)
     return VEGAS_OK;
 }
 
+int vegas_combine_iterations(int n, const double* I, const double* sg, double* mean, double* comb_error, double* chi2_dof)
+{
+    if (n < 1 || !I || !sg || !mean || !comb_error) return fail(VEGAS_EINVAL, "combine: n >= 1 and non-NULL arrays/outputs required");
+    double sw = 0.0, swi = 0.0, plain = 0.0;
+    for (int i = 0; i < n; ++i) {
+        plain += I[i];
+        if (sg[i] > 0.0 && std::isfinite(sg[i]) && std::isfinite(I[i])) {
+            const double w = 1.0 / (sg[i] * sg[i]);
+            sw += w;
+            swi += w * I[i];
+        }
+    }
+    if (!(sw > 0.0)) {                                   // no iteration carries weight
+        *mean = plain / n;
+        *comb_error = 0.0;
+        if (chi2_dof) *chi2_dof = 0.0;
+        return VEGAS_OK;
+    }
+    const double m = swi / sw;
+    double chi2 = 0.0;
+    for (int i = 0; i < n; ++i)
+        if (sg[i] > 0.0 && std::isfinite(sg[i]) && std::isfinite(I[i])) {
+            const double dlt = I[i] - m;
+            chi2 += dlt * dlt / (sg[i] * sg[i]);
+        }
+    *mean = m;
+    *comb_error = 1.0 / std::sqrt(sw);
+    if (chi2_dof) *chi2_dof = (n > 1) ? chi2 / (n - 1) : 0.0;
+    return VEGAS_OK;
+}
+
+int vegas_run_integration(vegas_ctx* c, int n_iter, int n_warmup, uint64_t n_events, uint64_t events_per_launch,
+                          uint64_t seed, double alpha, double* mean, double* error, double* chi2_dof,
+                          double* iter_integral, double* iter_error, double* iter_kernel_ms)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (n_iter < 1 || n_warmup < 0) return fail(VEGAS_EINVAL, "n_iter >= 1 and n_warmup >= 0 required");
+    if (!mean || !error) return fail(VEGAS_EINVAL, "mean and error are required");
+    const int total = n_warmup + n_iter;
+    double* I = static_cast<double*>(std::malloc(sizeof(double) * 2 * static_cast<size_t>(total)));
+    if (!I) return fail(VEGAS_ENOMEM, "host allocation failed");
+    double* sg = I + total;
+    int rc = VEGAS_OK;
+    for (int it = 0; it < total && rc == VEGAS_OK; ++it) {
+        rc = vegas_iterate(c, n_events, events_per_launch, seed, &I[it], &sg[it], nullptr);
+        if (rc != VEGAS_OK) break;
+        if (iter_kernel_ms) rc = vegas_last_sums(c, nullptr, nullptr, &iter_kernel_ms[it]);
+        if (rc != VEGAS_OK) break;
+        rc = vegas_refine(c, alpha);
+        if (rc == VEGAS_EGRID) rc = VEGAS_OK;            // grid unchanged; keep integrating
+    }
+    if (rc == VEGAS_OK) {
+        if (iter_integral) std::memcpy(iter_integral, I, sizeof(double) * total);
+        if (iter_error) std::memcpy(iter_error, sg, sizeof(double) * total);
+        rc = vegas_combine_iterations(n_iter, I + n_warmup, sg + n_warmup, mean, error, chi2_dof);
+    }
+    std::free(I);
+    return rc;
+}
+
 int vegas_get_grid(const vegas_ctx* c, double* edges)
 {
     if (!c || !edges) return fail(VEGAS_EINVAL, "NULL argument");

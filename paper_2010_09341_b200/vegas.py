@@ -41,6 +41,9 @@ SIGNATURES = {
     "vegas_get_launch_shape": (C.c_int, [_vp, _ip, _ip, _ip, _szp]),
     "vegas_device_info": (C.c_int, [_vp, _ip, _ip]),
     "vegas_pipe_rate": (C.c_int, [C.c_int, _vp, _dp]),
+    "vegas_run_integration": (C.c_int, [_vp, C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, _dp, _dp,
+                                        _dp, _dp, _dp, _dp]),
+    "vegas_combine_iterations": (C.c_int, [C.c_int, _dp, _dp, _dp, _dp, _dp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
 }
@@ -127,6 +130,18 @@ class Vegas:
     def refine(self, alpha):
         _chk(lib().vegas_refine(self._h, float(alpha)), "vegas_refine")
 
+    def run_integration(self, n_iter, n_events, events_per_launch=0, seed=0, alpha=1.5, n_warmup=0):
+        """PAPER.md:L79 run_integration: returns (mean, error, chi2_dof, per-iteration dict)."""
+        n_events = int(n_events)
+        epl = int(events_per_launch) if events_per_launch else n_events
+        tot = n_iter + n_warmup
+        m, e, c2 = C.c_double(), C.c_double(), C.c_double()
+        I, s, ms = np.empty(tot), np.empty(tot), np.empty(tot)
+        _chk(lib().vegas_run_integration(self._h, int(n_iter), int(n_warmup), n_events, epl, int(seed), float(alpha),
+                                         C.byref(m), C.byref(e), C.byref(c2), _d(I), _d(s), _d(ms)),
+             "vegas_run_integration")
+        return m.value, e.value, c2.value, dict(integral=I, error=s, kernel_ms=ms)
+
     # ---- asynchronous form (timing) ------------------------------------------------------------------
     def iterate_enqueue(self, n_events, events_per_launch=0, seed=0):
         n_events = int(n_events)
@@ -211,6 +226,17 @@ def pipe_rate(pipe, stream=None):
     _chk(lib().vegas_pipe_rate(int(pipe), _vp(stream.cuda_stream) if stream is not None else None, C.byref(v)),
          "vegas_pipe_rate")
     return v.value
+
+
+def combine_iterations(integral, error):
+    """Inverse-variance combination of iteration estimates (vegas_combine_iterations; host arithmetic, no GPU)."""
+    I = np.ascontiguousarray(integral, dtype=np.float64)
+    s = np.ascontiguousarray(error, dtype=np.float64)
+    assert I.shape == s.shape and I.ndim == 1
+    m, e, c2 = C.c_double(), C.c_double(), C.c_double()
+    _chk(lib().vegas_combine_iterations(int(I.size), _d(I), _d(s), C.byref(m), C.byref(e), C.byref(c2)),
+         "vegas_combine_iterations")
+    return m.value, e.value, c2.value
 
 
 def from_workload(w, **kw):
