@@ -20,7 +20,9 @@ namespace {
 
 using namespace vegas;
 
-constexpr int kMaxSlots = 4096;          // upper bound on the iterate grid (CTAs)
+constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
+constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the iterate grid (CTAs)
+constexpr int kMaxSlots = kLanes * kLaneSlots;
 constexpr double kPi = 0x1.921fb54442d18p+1;   // fl64(pi)
 
 thread_local char g_err[512] = "";
@@ -195,6 +197,8 @@ struct vegas_ctx {
     double* h_result;        // pinned: result[8] then hist[dim*nbins]
     int* h_status;           // pinned
     cudaEvent_t ev0, ev1;
+    cudaStream_t lane[kLanes];       // non-blocking streams: small launches of one iteration overlap on the GPU
+    cudaEvent_t lane_done[kLanes], fork;
     uint64_t last_n;
     int last_launches;
 };
@@ -282,7 +286,7 @@ int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
     CUDA_TRY(in->occupancy(&occ, threads, smem));
     if (occ < 1) return fail(VEGAS_EINVAL, "launch shape (%d threads, %zu B smem) cannot run", threads, smem);
     if (occ < ctas) ctas = occ;
-    if (ctas * c->sm_count > kMaxSlots) ctas = kMaxSlots / c->sm_count;
+    if (ctas * c->sm_count > kLaneSlots) ctas = kLaneSlots / c->sm_count;
     c->inst = in;
     c->ctas_per_sm = ctas; c->threads = threads; c->rshift = rshift; c->smem_bytes = smem;
     return VEGAS_OK;
@@ -307,6 +311,15 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
     a.nbins = c->nbins;
     a.rshift = c->rshift;
     a.ic = c->ic;
+}
+
+bool create_lanes(vegas_ctx* c)
+{
+    for (int i = 0; i < kLanes; ++i)
+        if (cudaStreamCreateWithFlags(&c->lane[i], cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->lane_done[i], cudaEventDisableTiming) != cudaSuccess)
+            return false;
+    return true;
 }
 
 int build_table(vegas_ctx* c, int uniform)
@@ -365,7 +378,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->ws = static_cast<unsigned char*>(dev_workspace);
     c->L = L;
     c->iteration = 0; c->have_hist = false; c->have_sums = false;
-    c->h_result = nullptr; c->h_status = nullptr; c->ev0 = nullptr; c->ev1 = nullptr;
+    c->h_result = nullptr; c->h_status = nullptr; c->ev0 = nullptr; c->ev1 = nullptr; c->fork = nullptr;
+    for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0;
     int rc = setup_integrand(c, params);
     if (rc != VEGAS_OK) { delete c; return rc; }
@@ -383,7 +397,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->sm_clock_khz = khz;
     if (cudaHostAlloc(reinterpret_cast<void**>(&c->h_result), (8 + static_cast<size_t>(dim) * nbins) * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
-        cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess)
+        cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) != cudaSuccess || !create_lanes(c))
         return cleanup(fail(VEGAS_ECUDA, "pinned host buffer / event creation failed: %s", cudaGetErrorString(cudaGetLastError())));
     rc = apply_shape(c, 0, 0, -1);
     if (rc != VEGAS_OK && c->tuned) { c->tuned = nullptr; rc = apply_shape(c, 0, 0, -1); }
@@ -404,6 +419,11 @@ void vegas_destroy(vegas_ctx* c)
     if (c->h_status) cudaFreeHost(c->h_status);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    if (c->fork) cudaEventDestroy(c->fork);
+    for (int i = 0; i < kLanes; ++i) {
+        if (c->lane[i]) cudaStreamDestroy(c->lane[i]);
+        if (c->lane_done[i]) cudaEventDestroy(c->lane_done[i]);
+    }
     delete c;
 }
 
@@ -456,6 +476,17 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
     IterArgs a;
     fill_args(c, seed, 0, 0, a);
     const int max_grid = c->ctas_per_sm * c->sm_count;
+    // Launches of one iteration are independent (global event index; the histogram and the pass counter are
+    // accumulated with global reductions; each lane has its own slot region), so when an iteration is cut into
+    // several launches they are dealt round-robin to kLanes internal streams forked from the caller's stream:
+    // launches that do not fill the GPU overlap, and every launch's prologue/flush overlaps its neighbours'.
+    const uint64_t n_launches = (n_events + epl - 1) / epl;
+    const int lanes = n_launches > 1 ? kLanes : 1;
+    if (lanes > 1) {
+        CUDA_TRY(cudaEventRecord(c->fork, c->stream));
+        for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
+    }
+    double* slots0 = reinterpret_cast<double*>(c->ws + c->L.slots);
     int launches = 0, used_grid = 0;
     for (uint64_t done = 0; done < n_events;) {
         uint64_t cnt = n_events - done;
@@ -467,12 +498,20 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
         a.count = static_cast<uint32_t>(cnt);
         const uint64_t want = (cnt + c->threads - 1) / c->threads;
         const int grid = want < static_cast<uint64_t>(max_grid) ? static_cast<int>(want) : max_grid;
-        CUDA_TRY(c->inst->launch(a, grid, c->threads, c->smem_bytes, c->stream));
+        const int ln = launches % lanes;
+        a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
+        CUDA_TRY(c->inst->launch(a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
         if (grid > used_grid) used_grid = grid;
         done += cnt;
         ++launches;
     }
-    finalize_kernel<<<1, 32, 0, c->stream>>>(reinterpret_cast<const double*>(c->ws + c->L.slots), used_grid,
+    if (lanes > 1) {
+        for (int i = 0; i < lanes; ++i) {
+            CUDA_TRY(cudaEventRecord(c->lane_done[i], c->lane[i]));
+            CUDA_TRY(cudaStreamWaitEvent(c->stream, c->lane_done[i], 0));
+        }
+    }
+    finalize_kernel<<<1, 32, 0, c->stream>>>(slots0, lanes, kLaneSlots, used_grid,
                                              reinterpret_cast<const unsigned long long*>(c->ws + c->L.npass),
                                              n_events, reinterpret_cast<double*>(c->ws + c->L.result));
     CUDA_TRY(cudaGetLastError());

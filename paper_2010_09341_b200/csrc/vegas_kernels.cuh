@@ -298,16 +298,19 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 // ------------------------------------------------------------------------------------------------
 // finalize_kernel (S6): fixed-order compensated sum of the per-CTA slots, then
 //   I = S1/n ; V = (S2/n - I*I)/(n-1) ; sigma = sqrt(max(V, 0)).
-// One warp; lane l folds slots l, l+32, ... then a shuffle tree: the order depends only on nslots.
+// One warp; lane l folds slots l, l+32, ... (over the per-stream-lane regions) then a shuffle tree: the order
+// depends only on the launch geometry.
 // result[0..5] = I, sigma, S1, S2, npass, n
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__ slots, int nslots,
+__global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__ slots, int nlanes, int lane_stride,
+                                                      int per_lane,
                                                       const unsigned long long* __restrict__ npass,
                                                       unsigned long long n_events, double* __restrict__ result)
 {
     const int lane = threadIdx.x;
     Comp t1{0.0, 0.0}, t2{0.0, 0.0};
-    for (int s = lane; s < nslots; s += 32) {
+    for (int e = lane; e < nlanes * per_lane; e += 32) {         // slot region of stream-lane e / per_lane
+        const size_t s = static_cast<size_t>(e / per_lane) * lane_stride + (e % per_lane);
         comp_add(t1, slots[s * 4 + 0], slots[s * 4 + 1]);
         comp_add(t2, slots[s * 4 + 2], slots[s * 4 + 3]);
     }
