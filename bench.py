@@ -36,7 +36,7 @@ UNIT = "events/s"
 # Algorithmic FP work per event (FMA = 2 FLOPs, exp/cos/div
 # expanded to the sequences nvcc emits).  fp64 FLOPs for the fp64 configs, fp32 FLOPs for cfg4.
 # cfg5: 130 per event that passes the cuts, 14 per rejected one (mean taken with the measured pass fraction).
-ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg4": 232.0, "cfg5": (130.0, 14.0)}
+ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg2_u32": 154.0, "cfg4": 232.0, "cfg5": (130.0, 14.0)}
 # FP pipe lanes per SM (B200): 64 fp64, 128 fp32.  Peak = SMs * lanes * 2 FLOP * max SM clock.
 FP_LANES = {"f64": 64, "f32": 128}
 # dram__bytes_read.sum + dram__bytes_write.sum of one 1e8-event iterate_kernel launch, from the ncu --set full
@@ -51,7 +51,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg4", "cfg5"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg1", "cfg2", "cfg4", "cfg5", "cfg2_u32"])
     ap.add_argument("--n-events", type=int, default=0, help="override events per iteration (parity/debug only)")
     ap.add_argument("--epl", type=int, default=0, help="events per launch (0 = whole iteration in one launch)")
     ap.add_argument("--ctas-per-sm", type=int, default=0)
@@ -70,7 +70,7 @@ def workload(args):
 
 
 def dtype_of(w):
-    return "f64" if w.precision == W.FP64 else "f32"
+    return "f32" if w.precision == W.FP32_EVAL else "f64"
 
 
 def config_of(args, w, n, shape=None):

@@ -47,7 +47,13 @@ enum {
 /* Per-event arithmetic precision (uniform, map, Jacobian, integrand).  wf, (wf)^2, all sums, the
  * histogram, the refinement and the master edges are always fp64 (BASELINE.json configs[3]: "FP32
  * integrand with FP64 accumulation"; reading R14). */
-enum { VEGAS_FP64 = 0, VEGAS_FP32_EVAL = 1 };
+enum { VEGAS_FP64 = 0, VEGAS_FP32_EVAL = 1,
+       /* fp64 arithmetic throughout, but one 32-bit Philox word per coordinate instead of 52 bits of two words
+        * (reading R3: "a 32-bit-per-coordinate variant ... as an extra, mirrored in the oracle and reported
+        * separately"): u = r/2^32, coordinate k uses block k>>2, word k&3.  Halves the Philox work of the fp64
+        * configurations; the estimates are those of a different, equally valid random stream.  Available for
+        * gauss_sym, gauss_double, lo_2to2 and toy_sum. */
+       VEGAS_FP64_U32 = 2 };
 
 /* Built-in integrands (device functions chosen at compile time; BASELINE.json north_star "Integrand
  * evaluation") and their `params` (doubles):

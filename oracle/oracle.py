@@ -26,7 +26,7 @@ _LIB = os.path.join(_HERE, "liboracle_vegas.so")
 CFLAGS = ["-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared"]
 
 OK, EINVAL, ENOMEM, ESTATE, EUNSUPPORTED, EGRID = 0, -1, -3, -4, -5, -6
-FP64, FP32_EVAL = 0, 1
+FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
 
 _lock = threading.Lock()
 _lib = None

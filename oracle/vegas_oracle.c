@@ -39,7 +39,11 @@
 
 enum { ORACLE_OK = 0, ORACLE_EINVAL = -1, ORACLE_ENOMEM = -3, ORACLE_ESTATE = -4,
        ORACLE_EUNSUPPORTED = -5, ORACLE_EGRID = -6 };
-enum { ORACLE_FP64 = 0, ORACLE_FP32_EVAL = 1 };
+enum { ORACLE_FP64 = 0, ORACLE_FP32_EVAL = 1, ORACLE_FP64_U32 = 2 };
+/* ORACLE_FP64_U32: fp64 arithmetic, one 32-bit Philox word per coordinate (B = 32): the extra stream mode of
+ * DESIGN.md reading R3.  is_f64() is true for both fp64 modes. */
+#define is_f64(c) ((c)->precision != ORACLE_FP32_EVAL)
+#define ubits(c) ((c)->precision == ORACLE_FP64 ? 52 : ((c)->precision == ORACLE_FP64_U32 ? 32 : 23))
 enum { ID_GAUSS_SYM = 0, ID_GAUSS_DOUBLE = 1, ID_GENZ_OSC_PEAK = 2, ID_LO_2TO2 = 3, ID_TOY_SUM = 4 };
 
 /* fl64(pi) = 3.141592653589793115997963... */
@@ -103,7 +107,12 @@ static void event_words(uint64_t seed, uint32_t it, uint64_t e, uint32_t j, uint
 void oracle_mantissas(const oracle_ctx *c, uint64_t seed, uint32_t it, uint64_t e, uint64_t *m)
 {
     uint32_t r[4];
-    if (c->precision == ORACLE_FP64) {
+    if (c->precision == ORACLE_FP64_U32) {                 /* m = r[k&3]: all 32 bits of one word */
+        for (int k = 0; k < c->dim; ++k) {
+            if ((k & 3) == 0) event_words(seed, it, e, (uint32_t)(k >> 2), r);
+            m[k] = (uint64_t)r[k & 3];
+        }
+    } else if (c->precision == ORACLE_FP64) {
         for (int k = 0; k < c->dim; ++k) {
             if ((k & 1) == 0) event_words(seed, it, e, (uint32_t)(k >> 1), r);
             int a = 2 * (k & 1);
@@ -201,7 +210,7 @@ static int setup_integrand(oracle_ctx *c)
     case ID_GAUSS_SYM:      /* params {alpha, mu} */
     case ID_GAUSS_DOUBLE: { /* params {alpha, mu1, mu2} */
         int need = (c->integrand_id == ID_GAUSS_SYM) ? 2 : 3;
-        if (c->n_params != need || c->precision != ORACLE_FP64) return ORACLE_EINVAL;
+        if (c->n_params != need || !is_f64(c)) return ORACLE_EINVAL;
         double alpha = p[0];
         double b = alpha * sqrt(ORACLE_PI);        /* b = fl(alpha*fl(sqrt(pi))) */
         double C = 1.0;
@@ -223,7 +232,7 @@ static int setup_integrand(oracle_ctx *c)
         return ORACLE_OK;
     }
     case ID_LO_2TO2: { /* params {sqrt_s, sqrt_shat_min, cos_cut, pdf_a, pdf_b}; pdf_b fixed = 5 */
-        if (c->n_params != 5 || c->dim != 3 || c->precision != ORACLE_FP64) return ORACLE_EINVAL;
+        if (c->n_params != 5 || c->dim != 3 || !is_f64(c)) return ORACLE_EINVAL;
         if (p[4] != 5.0) return ORACLE_EUNSUPPORTED;
         double s = p[0] * p[0];
         double smin = p[1] * p[1];
@@ -248,9 +257,9 @@ int oracle_create(oracle_ctx **out, int dim, int nbins, int integrand_id, const 
     if (!out || dim < 1 || dim > ORACLE_MAX_DIM || nbins < 2 || n_params < 0 ||
         n_params > ORACLE_MAX_PARAMS || (n_params > 0 && !params))
         return ORACLE_EINVAL;
-    if (precision != ORACLE_FP64 && precision != ORACLE_FP32_EVAL) return ORACLE_EINVAL;
+    if (precision != ORACLE_FP64 && precision != ORACLE_FP32_EVAL && precision != ORACLE_FP64_U32) return ORACLE_EINVAL;
     /* p=m*N must fit: N<2^12 with 52-bit m, N<2^9 with 23-bit m (S2) */
-    if ((precision == ORACLE_FP64 && nbins >= 4096) || (precision == ORACLE_FP32_EVAL && nbins >= 512))
+    if ((precision != ORACLE_FP32_EVAL && nbins >= 4096) || (precision == ORACLE_FP32_EVAL && nbins >= 512))
         return ORACLE_EINVAL;
     oracle_ctx *c = (oracle_ctx *)calloc(1, sizeof(oracle_ctx));
     if (!c) return ORACLE_ENOMEM;
@@ -404,13 +413,14 @@ static void map_eval(const oracle_ctx *c, const uint64_t *m, int32_t *bins, doub
                      double *fo, double *wfo, int *passo)
 {
     const int d = c->dim, N = c->nbins;
-    if (c->precision == ORACLE_FP64) {
+    if (is_f64(c)) {
+        const int B = ubits(c);                                   /* 52, or 32 in the 32-bit-uniform mode */
         double x[ORACLE_MAX_DIM];
         double J = 0.0;
         for (int k = 0; k < d; ++k) {
-            uint64_t p = m[k] * (uint64_t)N;                       /* exact: m<2^52, N<2^12 */
-            int i = (int)(p >> 52);
-            double frac = ldexp((double)(p & ((1ull << 52) - 1)), -52);   /* exact */
+            uint64_t p = m[k] * (uint64_t)N;                       /* exact: m<2^B<=2^52, N<2^12 */
+            int i = (int)(p >> B);
+            double frac = ldexp((double)(p & ((1ull << B) - 1)), -B);     /* exact */
             size_t t = (size_t)k * N + i;
             x[k] = fma(frac, c->wd_d[t], c->lo_d[t]);
             J = (k == 0) ? c->g_d[t] : J * c->g_d[t];
@@ -469,7 +479,7 @@ int oracle_map_eval(const oracle_ctx *c, const uint64_t *m, uint32_t count, int3
     if (!c || !m) return ORACLE_EINVAL;
     int32_t b[ORACLE_MAX_DIM];
     double xx[ORACLE_MAX_DIM];
-    const uint64_t lim = (c->precision == ORACLE_FP64) ? (1ull << 52) : (1ull << 23);
+    const uint64_t lim = 1ull << ubits(c);
     for (uint32_t n = 0; n < count; ++n) {
         double J, fv, w; int ps;
         for (int k = 0; k < c->dim; ++k)
@@ -645,7 +655,7 @@ int oracle_get_table(const oracle_ctx *c, double *lo, double *wd, double *g)
     if (!c) return ORACLE_EINVAL;
     size_t cells = (size_t)c->dim * c->nbins;
     for (size_t t = 0; t < cells; ++t) {
-        if (c->precision == ORACLE_FP64) {
+        if (is_f64(c)) {
             if (lo) lo[t] = c->lo_d[t];
             if (wd) wd[t] = c->wd_d[t];
             if (g) g[t] = c->g_d[t];

@@ -136,6 +136,7 @@ const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, 50, 5, 8, 8, VEGAS_FP64, 1024, 1, 1024),      // configs[1], [2]
     VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 0, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
     VEGAS_TUNED(VEGAS_LO_2TO2, Lo2to2, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),                // configs[4]
+    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, U32<GaussDouble>, 8, 50, 5, 8, 8, VEGAS_FP64_U32, 1024, 1, 1024),   // configs[1] with 32-bit uniforms
     VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL),
@@ -146,6 +147,10 @@ const Instance kInstances[] = {
     VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 0, VEGAS_FP32_EVAL),
     VEGAS_GENERIC(VEGAS_TOY_SUM, ToySum<double>, 0, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_TOY_SUM, ToySum<float>, 0, VEGAS_FP32_EVAL),
+    VEGAS_GENERIC(VEGAS_GAUSS_SYM, U32<GaussSym>, 0, VEGAS_FP64_U32),
+    VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, U32<GaussDouble>, 0, VEGAS_FP64_U32),
+    VEGAS_GENERIC(VEGAS_LO_2TO2, U32<Lo2to2>, 3, VEGAS_FP64_U32),
+    VEGAS_GENERIC(VEGAS_TOY_SUM, U32<ToySum<double>>, 0, VEGAS_FP64_U32),
 };
 
 // The tuned instance for exactly (id, dim, nbins, precision), or NULL.
@@ -251,7 +256,7 @@ int setup_integrand(vegas_ctx* c, const double* p)
 size_t iterate_smem_bytes(const vegas_ctx* c, const Instance* in, int rshift, int threads)
 {
     const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
-    const size_t cell_bytes = (c->precision == VEGAS_FP64) ? 16 : 8;
+    const size_t cell_bytes = (c->precision == VEGAS_FP32_EVAL) ? 8 : 16;
     return align_up(cells * (size_t(1) << rshift) * 8, 16) + align_up(cells * in->trep * cell_bytes, 16) +
            static_cast<size_t>((threads + 31) / 32) * (5 * 8 + static_cast<size_t>(in->queue_entry_bytes) * kQueueCap);
 }
@@ -325,7 +330,7 @@ bool create_lanes(vegas_ctx* c)
 int build_table(vegas_ctx* c, int uniform)
 {
     build_table_kernel<<<c->dim, 128, 0, c->stream>>>(reinterpret_cast<double*>(c->ws + c->L.edges),
-                                                      c->ws + c->L.table, c->nbins, c->precision, uniform);
+                                                      c->ws + c->L.table, c->nbins, c->precision == VEGAS_FP32_EVAL ? 1 : 0, uniform);
     CUDA_TRY(cudaGetLastError());
     return VEGAS_OK;
 }
@@ -351,8 +356,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     if (!out) return fail(VEGAS_EINVAL, "out is NULL");
     *out = nullptr;
     if (dim < 1 || dim > kMaxDim) return fail(VEGAS_EINVAL, "dim %d not in 1..%d", dim, kMaxDim);
-    if (precision != VEGAS_FP64 && precision != VEGAS_FP32_EVAL) return fail(VEGAS_EINVAL, "precision %d unknown", precision);
-    const int max_bins = (precision == VEGAS_FP64) ? 4095 : 511;     // m*N must be exact (S2)
+    if (precision != VEGAS_FP64 && precision != VEGAS_FP32_EVAL && precision != VEGAS_FP64_U32) return fail(VEGAS_EINVAL, "precision %d unknown", precision);
+    const int max_bins = (precision == VEGAS_FP32_EVAL) ? 511 : 4095;     // m*N must be exact (S2)
     if (nbins < 2 || nbins > max_bins) return fail(VEGAS_EINVAL, "nbins %d not in 2..%d", nbins, max_bins);
     const int need = expected_params(integrand_id, dim);
     if (need < 0) return fail(VEGAS_EUNSUPPORTED, "integrand_id %d unknown", integrand_id);
@@ -592,7 +597,7 @@ int vegas_refine(vegas_ctx* c, double alpha)
     refine_kernel<<<c->dim, 128, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags);
     CUDA_TRY(cudaGetLastError());
     refine_commit_kernel<<<c->dim, 128, 0, c->stream>>>(edges, new_edges, flags, c->dim, N, c->ws + c->L.table,
-                                                        c->precision, hist, status);
+                                                        c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status);
     CUDA_TRY(cudaGetLastError());
     CUDA_TRY(cudaMemcpyAsync(c->h_status, status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));

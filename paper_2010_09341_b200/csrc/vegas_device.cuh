@@ -91,6 +91,15 @@ __device__ __forceinline__ void bin_frac64(uint32_t w_lo, uint32_t w_hi, uint32_
     frac = __dadd_rn(__hiloint2double(static_cast<int>(fh), static_cast<int>(static_cast<uint32_t>(p))), -1.0);
 }
 
+// 32-bit-uniform stream mode (VEGAS_FP64_U32): m = w (32 bits), p = m*N, i = p>>32, frac = (p mod 2^32)/2^32.
+__device__ __forceinline__ void bin_frac64_u32(uint32_t w, uint32_t N, int& i, double& frac)
+{
+    const uint64_t p = static_cast<uint64_t>(w) * static_cast<uint64_t>(N);
+    const uint32_t lo = static_cast<uint32_t>(p);
+    i = static_cast<int>(p >> 32);
+    frac = __dadd_rn(__hiloint2double(static_cast<int>(0x3FF00000u | (lo >> 12)), static_cast<int>(lo << 20)), -1.0);
+}
+
 __device__ __forceinline__ void bin_frac32(uint32_t w, uint32_t N, int& i, float& frac)
 {
     const uint32_t p = (w >> 9) * N;
@@ -106,6 +115,7 @@ __device__ __forceinline__ void bin_frac32(uint32_t w, uint32_t N, int& i, float
 struct GaussSym {            // I0, BASELINE.json configs[0]
     using real = double;
     static constexpr int kId = 0;
+    static constexpr bool kU32 = false;
     static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     double s;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { s = 0.0; }
@@ -124,6 +134,7 @@ struct GaussSym {            // I0, BASELINE.json configs[0]
 struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
     using real = double;
     static constexpr int kId = 1;
+    static constexpr bool kU32 = false;
     static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     double s1, s2;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { s1 = 0.0; s2 = 0.0; }
@@ -171,6 +182,7 @@ __device__ __forceinline__ float cos_f32(float a)
 struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event arithmetic
     using real = float;
     static constexpr int kId = 2;
+    static constexpr bool kU32 = false;
     static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     float arg, Q;
     __device__ __forceinline__ void begin(const IntegrandConsts& c) { arg = c.zphi; Q = 1.0f; }
@@ -191,6 +203,7 @@ struct GenzOscPeak {         // I2, BASELINE.json configs[3], fp32 per-event ari
 struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, v3)
     using real = double;
     static constexpr int kId = 3;
+    static constexpr bool kU32 = false;
     static constexpr bool kHasCut = true;   // true: f = 0 for events the integrand's cuts reject
     double v[3];
     __device__ __forceinline__ void begin(const IntegrandConsts&) {}
@@ -234,6 +247,7 @@ template <typename Real>
 struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1)
     using real = Real;
     static constexpr int kId = 4;
+    static constexpr bool kU32 = false;
     static constexpr bool kHasCut = false;   // true: f = 0 for events the integrand's cuts reject
     Real f;
     __device__ __forceinline__ void begin(const IntegrandConsts&) { f = Real(0); }
@@ -243,6 +257,13 @@ struct ToySum {              // I4: tf.reduce_sum(xarr, axis=1
     }
     __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
     __device__ __forceinline__ Real end(const IntegrandConsts&, int) const { return f; }
+};
+
+// The same fp64 integrand driven by the 32-bit-uniform stream (VEGAS_FP64_U32).
+template <class F>
+struct U32 : F {
+    static_assert(sizeof(typename F::real) == 8, "U32 wraps fp64 integrands");
+    static constexpr bool kU32 = true;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -270,10 +291,16 @@ __device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint3
 #pragma unroll
         for (int k = 0; k < (D ? D : kMaxDim); ++k) {
             if (!D && k >= d) break;
-            if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 1), a, r);
-            const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
             int i; double frac;
-            bin_frac64(w_lo, w_hi, N, i, frac);
+            if constexpr (F::kU32) {                     // one 32-bit word per coordinate, four per Philox block
+                if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 2), a, r);
+                const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
+                bin_frac64_u32(w, N, i, frac);
+            } else {                                     // 52 bits of two words per coordinate
+                if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 1), a, r);
+                const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
+                bin_frac64(w_lo, w_hi, N, i, frac);
+            }
             const double2 t = tab[(k * static_cast<int>(N) + i) * TSTRIDE + toff];
             const double x = __fma_rn(frac, t.y, t.x);
             const double g = __dmul_rn(Nd, t.y);

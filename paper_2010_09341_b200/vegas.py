@@ -14,7 +14,7 @@ import numpy as np
 from . import build as _build
 
 OK, EINVAL, ECUDA, ENOMEM, ESTATE, EUNSUPPORTED, EGRID = 0, -1, -2, -3, -4, -5, -6
-FP64, FP32_EVAL = 0, 1
+FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
 GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM = 0, 1, 2, 3, 4
 
 _vp, _dp, _ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)

@@ -18,7 +18,7 @@ from typing import Tuple
 
 # integrand ids and precisions of the C ABI (include/vegas_b200.h)
 GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM = 0, 1, 2, 3, 4
-FP64, FP32_EVAL = 0, 1
+FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
 
 _M32 = 0xFFFFFFFF
 
@@ -71,6 +71,13 @@ def cfg2(n_events=10**8, n_iter=10):
                     n_events, n_iter, note="BASELINE.json configs[1] (headline)")
 
 
+def cfg2_u32(n_events=10**8, n_iter=10):
+    """configs[1] driven by the 32-bit-uniform stream (precision FP64_U32): an extra mode, reported separately."""
+    w = cfg2(n_events, n_iter)
+    return Workload("cfg2_gauss_double_d8_u32", w.dim, w.nbins, w.integrand_id, w.params, FP64_U32, n_events, n_iter,
+                    note="BASELINE.json configs[1] with 32-bit uniforms (extra mode, DESIGN.md R3)")
+
+
 def cfg3():
     w = cfg2(10**8, 5)
     return Workload("cfg3_batch_sweep_d8", w.dim, w.nbins, w.integrand_id, w.params, w.precision, 10**8, 5,
@@ -93,4 +100,4 @@ def toy(dim=10):
                     note="PAPER.md:L72-L79 usage example")
 
 
-ALL = {"cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5, "toy": toy}
+ALL = {"cfg1": cfg1, "cfg2": cfg2, "cfg2_u32": cfg2_u32, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5, "toy": toy}

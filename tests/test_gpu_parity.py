@@ -39,6 +39,11 @@ def small_workloads():
         "genz_d7": W.cfg4(dim=7),
         "toy_d32": W.Workload("toy32", 32, 50, W.TOY_SUM, (), W.FP64, 10**5, 3),
         "toy_f32_d9": W.Workload("toyf9", 9, 100, W.TOY_SUM, (), W.FP32_EVAL, 10**5, 3),
+        # 32-bit-uniform stream mode (extra; reading R3): tuned and generic instances
+        "cfg2_u32": W.cfg2_u32(),
+        "lo_u32": W.Workload("lo_u32", 3, 50, W.LO_2TO2, (13000.0, 50.0, 0.9, 1.1, 5.0), W.FP64_U32, 10**5, 3),
+        "gauss_sym_d5_u32": W.Workload("gs5u", 5, 33, W.GAUSS_SYM, (0.1, 0.5), W.FP64_U32, 10**5, 3),
+        "toy_d7_u32": W.Workload("toy7u", 7, 50, W.TOY_SUM, (), W.FP64_U32, 10**5, 3),
     }
 
 
@@ -86,7 +91,7 @@ def test_events_uniform_grid(V, O, name):
     assert_events_equal(g.debug_events(1000, 2000, seed=0xDEADBEEF12345678), o.events(1000, 2000, 0xDEADBEEF12345678), w)
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg4", "cfg5", "gauss_double_d5"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg4", "cfg5", "gauss_double_d5", "cfg2_u32"])
 def test_events_adapted_grid(V, O, name):
     """Cascade-free: load the oracle's refined grid into the library, then compare events."""
     w = small_workloads()[name]
@@ -175,7 +180,7 @@ def test_cfg1_full_five_iterations(V, O):
     run_cascade(g, o, w, w.n_events, w.n_iter)
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "toy", "gauss_sym_d2", "toy_f32_d9"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "toy", "gauss_sym_d2", "toy_f32_d9", "cfg2_u32", "lo_u32"])
 def test_cascade_reduced(V, O, name):
     w = small_workloads()[name]
     g, o = make_pair(V, O, w)
@@ -309,7 +314,7 @@ def test_estimates_within_4_sigma_of_closed_form(V, golden_dir):
 # BASELINE.json full sizes, in the launch configuration bench.py times (one launch per iteration, the
 # instance's default shape)
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "cfg2_u32"])
 def test_full_size_iteration_parity(V, O, name):
     """1e8 events: iteration 0 on the uniform grid and iteration 1 on the oracle's refined grid
     (cascade-free), I / sigma rel 1e-12, every histogram cell rel 1e-10, pass count exact, plus sampled events
