@@ -168,6 +168,17 @@ int vegas_run_integration(vegas_ctx* ctx, int n_iter, int n_warmup, uint64_t n_e
 int vegas_combine_iterations(int n, const double* integral, const double* error, double* mean, double* comb_error,
                              double* chi2_dof);
 
+/* Batch-size study / tuner (BASELINE.json north_star "Batching: the events-per-launch batch size is tuned on one
+ * GPU, mirroring the paper's batch-size study", "finding the right batch size can make a
+ * notable difference").  Times one iteration of n_events on the current grid for each of the n_candidates values
+ * of events_per_launch (after one untimed warm-up iteration; CUDA events around memset + launches + finalize),
+ * writes the times to ms[n_candidates] (host, may be NULL) and the fastest candidate to *best.  The grid and the
+ * iteration counter are left as they were; the device histogram afterwards belongs to a tuning run, so
+ * vegas_refine needs a fresh vegas_iterate (VEGAS_ESTATE otherwise).
+ * Errors: VEGAS_EINVAL (NULL candidates/best, n_candidates < 1, a candidate of 0, n_events < 2), VEGAS_ECUDA. */
+int vegas_tune_events_per_launch(vegas_ctx* ctx, uint64_t n_events, uint64_t seed, const uint64_t* candidates,
+                                 int n_candidates, uint64_t* best, double* ms);
+
 /* Measured instruction throughput (thread-instructions per second over the whole GPU, current clocks) of
  * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports
  * (BASELINE.json north_star: "fraction of the FP pipe roofline").  Each call runs a

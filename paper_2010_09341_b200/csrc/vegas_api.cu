@@ -606,6 +606,31 @@ int vegas_refine(vegas_ctx* c, double alpha)
     return VEGAS_OK;
 }
 
+int vegas_tune_events_per_launch(vegas_ctx* c, uint64_t n_events, uint64_t seed, const uint64_t* candidates,
+                                 int n_candidates, uint64_t* best, double* ms)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!candidates || !best || n_candidates < 1) return fail(VEGAS_EINVAL, "candidates, best and n_candidates >= 1 are required");
+    const uint32_t it0 = c->iteration;
+    int rc = VEGAS_OK;
+    double best_ms = 0.0;
+    for (int i = 0; i < n_candidates && rc == VEGAS_OK; ++i) {
+        double t = 0.0;
+        for (int rep = 0; rep < 2 && rc == VEGAS_OK; ++rep) {        // rep 0 warms up this launch geometry
+            c->iteration = it0;
+            rc = vegas_iterate_enqueue(c, n_events, candidates[i], seed, nullptr);
+            if (rc == VEGAS_OK) rc = vegas_last_sums(c, nullptr, nullptr, &t);
+        }
+        if (rc != VEGAS_OK) break;
+        if (ms) ms[i] = t;
+        if (i == 0 || t < best_ms) { best_ms = t; *best = candidates[i]; }
+    }
+    c->iteration = it0;
+    c->have_hist = false;
+    c->have_sums = false;
+    return rc;
+}
+
 int vegas_combine_iterations(int n, const double* I, const double* sg, double* mean, double* comb_error, double* chi2_dof)
 {
     if (n < 1 || !I || !sg || !mean || !comb_error) return fail(VEGAS_EINVAL, "combine: n >= 1 and non-NULL arrays/outputs required");

@@ -18,10 +18,14 @@ from . import vegas as V
 from . import workloads as W
 
 
-def run_config(name, w, n_iter=None, epl=0):
+def run_config(name, w, n_iter=None, epl=0, tune=False):
     g = V.from_workload(w)
     n_iter = n_iter or w.n_iter
     g.iterate(w.n_events, epl, w.seed)          # untimed warm-up on the uniform grid
+    tuned = None
+    if tune and w.n_events >= 10**6:
+        cands = [c for c in (10**4, 10**5, 10**6, 10**7, 10**8) if c <= w.n_events]
+        tuned = g.tune_events_per_launch(w.n_events, cands, seed=w.seed)
     g.reset()
     ms, wall, res, passf = [], [], [], []
     for _ in range(n_iter):
@@ -37,7 +41,8 @@ def run_config(name, w, n_iter=None, epl=0):
            "events_per_s_median": w.n_events / (statistics.median(ms) * 1e-3),
            "events_per_s_best": w.n_events / (min(ms) * 1e-3),
            "wall_ms_median": statistics.median(wall), "launch_shape": g.launch_shape(),
-           "pass_fraction_first_last": [passf[0], passf[-1]], "last_result": res[-1]}
+           "pass_fraction_first_last": [passf[0], passf[-1]], "last_result": res[-1],
+           "tuned_events_per_launch": tuned[0] if tuned else None, "tune_ms": tuned[1] if tuned else None}
     g.close()
     return out
 
@@ -58,7 +63,7 @@ def main():
                 rows.append(run_config("cfg3/epl=%d" % epl, w, epl=epl))
                 print(json.dumps(rows[-1]))
         else:
-            rows.append(run_config(name, w, epl=w.events_per_launch))
+            rows.append(run_config(name, w, epl=w.events_per_launch, tune=True))
             print(json.dumps(rows[-1]))
     if args.json:
         with open(args.json, "w") as f:

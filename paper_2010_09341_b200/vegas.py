@@ -43,6 +43,7 @@ SIGNATURES = {
     "vegas_pipe_rate": (C.c_int, [C.c_int, _vp, _dp]),
     "vegas_run_integration": (C.c_int, [_vp, C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, _dp, _dp,
                                         _dp, _dp, _dp, _dp]),
+    "vegas_tune_events_per_launch": (C.c_int, [_vp, C.c_uint64, C.c_uint64, _u64p, C.c_int, _u64p, _dp]),
     "vegas_combine_iterations": (C.c_int, [C.c_int, _dp, _dp, _dp, _dp, _dp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
@@ -141,6 +142,15 @@ class Vegas:
                                          C.byref(m), C.byref(e), C.byref(c2), _d(I), _d(s), _d(ms)),
              "vegas_run_integration")
         return m.value, e.value, c2.value, dict(integral=I, error=s, kernel_ms=ms)
+
+    def tune_events_per_launch(self, n_events, candidates, seed=0):
+        """The batch-size study of PAPER.md:L57-L65 on this GPU: (best candidate, {candidate: ms})."""
+        cand = (C.c_uint64 * len(candidates))(*[int(v) for v in candidates])
+        best = C.c_uint64()
+        ms = np.empty(len(candidates))
+        _chk(lib().vegas_tune_events_per_launch(self._h, int(n_events), int(seed), cand, len(candidates),
+                                                C.byref(best), _d(ms)), "vegas_tune_events_per_launch")
+        return int(best.value), {int(k): float(v) for k, v in zip(candidates, ms)}
 
     # ---- asynchronous form (timing) ------------------------------------------------------------------
     def iterate_enqueue(self, n_events, events_per_launch=0, seed=0):

@@ -360,3 +360,20 @@ def test_batch_size_study_shape(V):
         ms[epl] = best
     assert ms[10**4] > 5 * ms[10**7], ms
     assert ms[10**6] >= 0.95 * ms[10**7] and ms[10**6] < 2.5 * ms[10**7], ms
+
+
+def test_tune_events_per_launch_leaves_state_alone_and_prefers_large_batches(V, O):
+    w = W.cfg2(n_events=10**7)
+    g, o = make_pair(V, O, w)
+    g.iterate(200_000, 0, w.seed); g.refine(w.alpha)
+    o.iterate(200_000, w.seed, threads=THREADS); o.refine(w.alpha)
+    grid, it = g.get_grid(), g.iteration
+    best, ms = g.tune_events_per_launch(w.n_events, [10**4, 10**5, 10**6, 10**7], seed=w.seed)
+    assert best in (10**6, 10**7) and ms[10**4] > ms[10**7] and all(v > 0 for v in ms.values())
+    np.testing.assert_array_equal(g.get_grid(), grid)
+    assert g.iteration == it
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(w.alpha)                               # the histogram on the device is a tuning run's
+    assert ei.value.code == V.ESTATE
+    g.set_grid(o.get_grid())
+    assert_iteration_close(g.iterate(300_000, best, w.seed), o.iterate(300_000, w.seed, threads=THREADS))
