@@ -82,6 +82,9 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
  * depend on it, reading R16).  Event e draws its point from Philox4x32-10 keyed by `seed` with counter
  * (e, iteration, coordinate block), maps it through the grid, evaluates the integrand, and the kernels
  * accumulate S1 = sum wf, S2 = sum (wf)^2 and H[k][bin_k] += (wf)^2.
+ * When the iteration is cut into several launches they are dealt to internal non-blocking streams forked from and
+ * joined to the context's stream (they are independent: global event index, reductions into H), so small launches
+ * overlap; seen from the caller everything is ordered on the context's stream.
  *   integral = S1/n, error = sqrt(max(0,(S2/n - I^2)/(n-1))); hist (may be NULL) receives dim*nbins
  *   doubles, row-major [k][i].  The histogram also stays on the device for vegas_refine.
  * On success the iteration counter increments by one.  Non-finite results are returned as they are.
@@ -129,7 +132,8 @@ int vegas_iterate_enqueue(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per
 int vegas_iterate_collect(vegas_ctx* ctx, double* integral, double* error, double* hist);
 
 /* Launch-shape tuning knobs of the iterate kernel (the batch-size / occupancy study):
- * CTAs per SM and threads per CTA (0 = library default 2 x 512; threads a multiple of 32, <= 1024), and
+ * CTAs per SM and threads per CTA (0 = the kernel instance's default, 1 x 1024 for the instances tuned to the
+ * BASELINE.json configurations and 2 x 512 for the generic ones; threads a multiple of 32, <= 1024), and
  * the number R of lane-indexed shared-memory histogram replicas (power of two 1..32; 0 = the largest
  * that fits).  Results do not depend on them beyond summation order.  VEGAS_EINVAL if the shape cannot
  * run (shared memory); ctas_per_sm is clamped to what the device can hold. */
