@@ -229,13 +229,14 @@ def run_b200(args):
 
     def step_async():
         nl = g.iterate_enqueue(n, epl, w.seed)
-        g.refine(w.alpha)                   # S7; returns after its 4-byte status read
+        g.refine_enqueue(w.alpha)           # S7, no host round trip; outcome collected after the timed region
         return nl + 2
 
     # ---- device-timed region ----
     g.reset()
     for _ in range(args.warmup):
         step_async()
+    g.refine_collect()
     sampler = ClockSampler(local)
     barrier()
     sampler.start()
@@ -244,11 +245,14 @@ def run_b200(args):
     ev0.record()
     for _ in range(args.steps):
         launches += step_async()
-        iter_ms += g.last_sums()[2]         # the library's own CUDA events around memset+launches+finalize
     ev1.record()
     barrier()
     clocks = sampler.stop()
     dev_ms = ev0.elapsed_time(ev1)
+    g.refine_collect()                      # VegasError(EGRID) if a refinement of the timed region was rejected
+    # the library's own CUDA events around each iteration's memset + launches + finalize (last 64 kept)
+    kept = min(args.steps, 64)
+    iter_ms = sum(g.iteration_kernel_ms(b) for b in range(kept)) * (args.steps / kept)
     I, s, _ = g.iterate_collect(want_hist=False)
     pass_fraction = g.last_npass() / float(n)
 

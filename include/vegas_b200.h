@@ -98,6 +98,19 @@ int vegas_iterate(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch,
  * strictly increasing: grid unchanged), VEGAS_ECUDA. */
 int vegas_refine(vegas_ctx* ctx, double alpha);
 
+/* Asynchronous form of vegas_refine: enqueue only (no host synchronisation); the outcome of all refinements
+ * enqueued since the last collect is read by vegas_refine_collect (VEGAS_EGRID if any of them was rejected --
+ * each rejected one left its grid unchanged -- else VEGAS_OK), which synchronises the stream.  vegas_refine =
+ * enqueue + collect.  vegas_iterate_enqueue + vegas_refine_enqueue make a whole step without a host round trip
+ * (bench.py's device-timed region). */
+int vegas_refine_enqueue(vegas_ctx* ctx, double alpha);
+int vegas_refine_collect(vegas_ctx* ctx);
+
+/* Device time (ms, CUDA events on the context's stream: memset + launches + finalize) of the iteration enqueued
+ * `back` iterations ago (0 = the latest).  The last 64 iterations keep their events.  Synchronises on that
+ * iteration's end event.  VEGAS_EINVAL if `back` is out of range. */
+int vegas_iteration_kernel_ms(const vegas_ctx* ctx, int back, double* kernel_ms);
+
 /* Master edges, fp64, dim*(nbins+1) doubles row-major [k][i].  set validates 0 = E0 < E1 < ... < EN = 1
  * (else VEGAS_EGRID, grid unchanged) and rebuilds the table with wd = E[i+1]-E[i] (S2). */
 int vegas_get_grid(const vegas_ctx* ctx, double* edges);

@@ -20,6 +20,7 @@ namespace {
 
 using namespace vegas;
 
+constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
 constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
 constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the iterate grid (CTAs)
 constexpr int kMaxSlots = kLanes * kLaneSlots;
@@ -201,7 +202,9 @@ struct vegas_ctx {
     size_t smem_bytes;
     double* h_result;        // pinned: result[8] then hist[dim*nbins]
     int* h_status;           // pinned
-    cudaEvent_t ev0, ev1;
+    cudaEvent_t evA[kEvPool], evB[kEvPool];   // pair (n % kEvPool) brackets the n-th enqueued iteration
+    uint64_t n_enqueued;             // iterations enqueued so far
+    int refine_pending;              // refinements enqueued and not yet collected
     cudaStream_t lane[kLanes];       // non-blocking streams: small launches of one iteration overlap on the GPU
     cudaEvent_t lane_done[kLanes], fork;
     uint64_t last_n;
@@ -318,6 +321,13 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
     a.ic = c->ic;
 }
 
+bool create_event_pool(vegas_ctx* c)
+{
+    for (int i = 0; i < kEvPool; ++i)
+        if (cudaEventCreate(&c->evA[i]) != cudaSuccess || cudaEventCreate(&c->evB[i]) != cudaSuccess) return false;
+    return true;
+}
+
 bool create_lanes(vegas_ctx* c)
 {
     for (int i = 0; i < kLanes; ++i)
@@ -383,7 +393,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->ws = static_cast<unsigned char*>(dev_workspace);
     c->L = L;
     c->iteration = 0; c->have_hist = false; c->have_sums = false;
-    c->h_result = nullptr; c->h_status = nullptr; c->ev0 = nullptr; c->ev1 = nullptr; c->fork = nullptr;
+    c->h_result = nullptr; c->h_status = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0;
+    for (int i = 0; i < kEvPool; ++i) { c->evA[i] = nullptr; c->evB[i] = nullptr; }
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0;
     int rc = setup_integrand(c, params);
@@ -402,7 +413,7 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->sm_clock_khz = khz;
     if (cudaHostAlloc(reinterpret_cast<void**>(&c->h_result), (8 + static_cast<size_t>(dim) * nbins) * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
-        cudaEventCreate(&c->ev0) != cudaSuccess || cudaEventCreate(&c->ev1) != cudaSuccess ||
+        !create_event_pool(c) ||
         cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) != cudaSuccess || !create_lanes(c))
         return cleanup(fail(VEGAS_ECUDA, "pinned host buffer / event creation failed: %s", cudaGetErrorString(cudaGetLastError())));
     rc = apply_shape(c, 0, 0, -1);
@@ -422,8 +433,10 @@ void vegas_destroy(vegas_ctx* c)
     if (!c) return;
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_status) cudaFreeHost(c->h_status);
-    if (c->ev0) cudaEventDestroy(c->ev0);
-    if (c->ev1) cudaEventDestroy(c->ev1);
+    for (int i = 0; i < kEvPool; ++i) {
+        if (c->evA[i]) cudaEventDestroy(c->evA[i]);
+        if (c->evB[i]) cudaEventDestroy(c->evB[i]);
+    }
     if (c->fork) cudaEventDestroy(c->fork);
     for (int i = 0; i < kLanes; ++i) {
         if (c->lane[i]) cudaStreamDestroy(c->lane[i]);
@@ -476,7 +489,8 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
     if (events_per_launch == 0) return fail(VEGAS_EINVAL, "events_per_launch must be > 0");
     if (n_events > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
     const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
-    CUDA_TRY(cudaEventRecord(c->ev0, c->stream));
+    const int evi = static_cast<int>(c->n_enqueued % kEvPool);
+    CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
     CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
     IterArgs a;
     fill_args(c, seed, 0, 0, a);
@@ -520,7 +534,8 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
                                              reinterpret_cast<const unsigned long long*>(c->ws + c->L.npass),
                                              n_events, reinterpret_cast<double*>(c->ws + c->L.result));
     CUDA_TRY(cudaGetLastError());
-    CUDA_TRY(cudaEventRecord(c->ev1, c->stream));
+    CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
+    c->n_enqueued += 1;
     c->iteration += 1;
     c->have_hist = true;
     c->have_sums = true;
@@ -565,7 +580,8 @@ int vegas_last_sums(const vegas_ctx* c, double* S1, double* S2, double* kernel_m
     if (S2) *S2 = c->h_result[3];
     if (kernel_ms) {
         float ms = 0.f;
-        CUDA_TRY(cudaEventElapsedTime(&ms, c->ev0, c->ev1));
+        const int evi = static_cast<int>((c->n_enqueued - 1) % kEvPool);
+        CUDA_TRY(cudaEventElapsedTime(&ms, c->evA[evi], c->evB[evi]));
         *kernel_ms = ms;
     }
     return VEGAS_OK;
@@ -581,7 +597,7 @@ int vegas_last_npass(const vegas_ctx* c, uint64_t* npass)
     return VEGAS_OK;
 }
 
-int vegas_refine(vegas_ctx* c, double alpha)
+int vegas_refine_enqueue(vegas_ctx* c, double alpha)
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
@@ -599,10 +615,45 @@ int vegas_refine(vegas_ctx* c, double alpha)
     refine_commit_kernel<<<c->dim, 128, 0, c->stream>>>(edges, new_edges, flags, c->dim, N, c->ws + c->L.table,
                                                         c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status);
     CUDA_TRY(cudaGetLastError());
-    CUDA_TRY(cudaMemcpyAsync(c->h_status, status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CUDA_TRY(cudaStreamSynchronize(c->stream));
-    if (c->h_status[0] != 0) return fail(VEGAS_EGRID, "refined edges are not strictly increasing; grid unchanged");
     c->have_hist = false;
+    c->refine_pending += 1;
+    return VEGAS_OK;
+}
+
+int vegas_refine_collect(vegas_ctx* c)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (c->refine_pending == 0) return VEGAS_OK;
+    int* status = reinterpret_cast<int*>(c->ws + c->L.status);
+    CUDA_TRY(cudaMemcpyAsync(c->h_status, status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int), c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));
+    const int pending = c->refine_pending;
+    c->refine_pending = 0;
+    if (c->h_status[0] != 0)
+        return fail(VEGAS_EGRID, "refined edges were not strictly increasing in at least one of the last %d refinement(s); that grid was left unchanged", pending);
+    return VEGAS_OK;
+}
+
+int vegas_refine(vegas_ctx* c, double alpha)
+{
+    int rc = vegas_refine_collect(c);                    // outcome of earlier asynchronous refinements first
+    if (rc != VEGAS_OK && rc != VEGAS_EGRID) return rc;
+    rc = vegas_refine_enqueue(c, alpha);
+    if (rc != VEGAS_OK) return rc;
+    return vegas_refine_collect(c);
+}
+
+int vegas_iteration_kernel_ms(const vegas_ctx* c, int back, double* kernel_ms)
+{
+    if (!c || !kernel_ms) return fail(VEGAS_EINVAL, "NULL argument");
+    if (back < 0 || back >= kEvPool || static_cast<uint64_t>(back) >= c->n_enqueued)
+        return fail(VEGAS_EINVAL, "back = %d: only the last min(%d, iterations so far) iterations keep their events", back, kEvPool);
+    const int evi = static_cast<int>((c->n_enqueued - 1 - back) % kEvPool);
+    CUDA_TRY(cudaEventSynchronize(c->evB[evi]));
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, c->evA[evi], c->evB[evi]));
+    *kernel_ms = ms;
     return VEGAS_OK;
 }
 

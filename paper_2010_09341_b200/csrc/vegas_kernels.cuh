@@ -445,7 +445,8 @@ __global__ void refine_kernel(const double* __restrict__ edges, const double* __
 }
 
 // commit (S7 step 7): if every dimension passed, the candidate edges become the master edges, the table
-// is rebuilt and H is cleared; otherwise nothing changes.  status[0] = 0 ok / 1 rejected.
+// is rebuilt and H is cleared; otherwise nothing changes.  status[0] is set to 1 on a rejection (sticky: the
+// host clears it when it collects the outcome of the refinements enqueued since).
 __global__ void refine_commit_kernel(double* __restrict__ edges, const double* __restrict__ new_edges,
                                      const int* __restrict__ flags, int d, int N, void* __restrict__ table,
                                      int precision, double* __restrict__ hist, int* __restrict__ status)
@@ -453,7 +454,7 @@ __global__ void refine_commit_kernel(double* __restrict__ edges, const double* _
     const int k = blockIdx.x;
     int bad = 0;
     for (int j = 0; j < d; ++j) bad |= flags[j];
-    if (threadIdx.x == 0 && k == 0) status[0] = bad;
+    if (threadIdx.x == 0 && k == 0 && bad) status[0] = 1;   // sticky until the host collects and clears it
     if (bad) return;
     double* E = edges + static_cast<size_t>(k) * (N + 1);
     const double* En = new_edges + static_cast<size_t>(k) * (N + 1);

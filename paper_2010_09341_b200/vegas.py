@@ -26,6 +26,9 @@ SIGNATURES = {
     "vegas_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
     "vegas_iterate": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp, _dp]),
     "vegas_refine": (C.c_int, [_vp, C.c_double]),
+    "vegas_refine_enqueue": (C.c_int, [_vp, C.c_double]),
+    "vegas_refine_collect": (C.c_int, [_vp]),
+    "vegas_iteration_kernel_ms": (C.c_int, [_vp, C.c_int, _dp]),
     "vegas_get_grid": (C.c_int, [_vp, _dp]),
     "vegas_set_grid": (C.c_int, [_vp, _dp]),
     "vegas_reset": (C.c_int, [_vp]),
@@ -159,6 +162,17 @@ class Vegas:
         nl = C.c_int()
         _chk(lib().vegas_iterate_enqueue(self._h, n_events, epl, int(seed), C.byref(nl)), "vegas_iterate_enqueue")
         return nl.value
+
+    def refine_enqueue(self, alpha):
+        _chk(lib().vegas_refine_enqueue(self._h, float(alpha)), "vegas_refine_enqueue")
+
+    def refine_collect(self):
+        _chk(lib().vegas_refine_collect(self._h), "vegas_refine_collect")
+
+    def iteration_kernel_ms(self, back=0):
+        v = C.c_double()
+        _chk(lib().vegas_iteration_kernel_ms(self._h, int(back), C.byref(v)), "vegas_iteration_kernel_ms")
+        return v.value
 
     def iterate_collect(self, want_hist=True):
         I, s = C.c_double(), C.c_double()

@@ -377,3 +377,27 @@ def test_tune_events_per_launch_leaves_state_alone_and_prefers_large_batches(V, 
     assert ei.value.code == V.ESTATE
     g.set_grid(o.get_grid())
     assert_iteration_close(g.iterate(300_000, best, w.seed), o.iterate(300_000, w.seed, threads=THREADS))
+
+
+def test_async_step_equals_blocking_step(V):
+    """vegas_iterate_enqueue + vegas_refine_enqueue (bench.py's device-timed step) against the blocking calls."""
+    w = W.cfg1()
+    a, b = V.from_workload(w), V.from_workload(w)
+    for _ in range(3):
+        a.iterate_enqueue(w.n_events, 30_000, w.seed)
+        a.refine_enqueue(w.alpha)
+        b.iterate(w.n_events, 30_000, w.seed)
+        b.refine(w.alpha)
+    a.refine_collect()
+    np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-15)
+    Ia, sa, ha = a.iterate(w.n_events, 0, w.seed)
+    Ib, sb, hb = b.iterate(w.n_events, 0, w.seed)
+    assert abs(Ia - Ib) <= 1e-13 * abs(Ib) and abs(sa - sb) <= 1e-12 * sb
+    assert all(a.iteration_kernel_ms(k) > 0 for k in range(4))
+    with pytest.raises(V.VegasError) as ei:
+        a.iteration_kernel_ms(4)
+    assert ei.value.code == V.EINVAL
+    with pytest.raises(V.VegasError) as ei:
+        a.refine_enqueue(w.alpha); a.refine_enqueue(w.alpha)       # second one has no histogram
+    assert ei.value.code == V.ESTATE
+    a.refine_collect()
