@@ -178,7 +178,13 @@ int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
  * iteration's estimate and device time (the `log_time` of the paper's call).  A refine that fails with
  * VEGAS_EGRID leaves the grid as it was and the run goes on.  The per-iteration work runs in the kernels; the
  * combination is host arithmetic over n_iter numbers (vegas_combine_iterations, callable on its own, no GPU).
+ * By default the whole step {memset, launches, finalize, refine, commit} is captured once into a CUDA graph and
+ * replayed (the iteration counter then lives in device memory and the per-iteration (I, sigma) are logged on the
+ * device; one host synchronisation per 64 iterations; iter_kernel_ms receives the average device time of a step,
+ * refinement included).  vegas_use_cuda_graph(ctx, 0) selects the plain loop of blocking calls (per-iteration
+ * times, refinement excluded).  Both give the same numbers.
  * Errors: VEGAS_EINVAL (n_iter < 1, n_warmup < 0, NULL mean/error, iterate's argument errors), VEGAS_ECUDA. */
+int vegas_use_cuda_graph(vegas_ctx* ctx, int enable);
 int vegas_run_integration(vegas_ctx* ctx, int n_iter, int n_warmup, uint64_t n_events, uint64_t events_per_launch,
                           uint64_t seed, double alpha, double* mean, double* error, double* chi2_dof,
                           double* iter_integral, double* iter_error, double* iter_kernel_ms);

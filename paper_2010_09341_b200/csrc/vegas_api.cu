@@ -20,6 +20,7 @@ namespace {
 
 using namespace vegas;
 
+constexpr int kRing = 64;               // (I, sigma) entries logged on the device between two reads of a graph run
 constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
 constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
 constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the iterate grid (CTAs)
@@ -48,7 +49,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ---- device workspace layout (all offsets 256-byte aligned) -------------------------------------
 struct Layout {
-    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, total;
+    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, dev_iter, ring, total;
 };
 
 Layout make_layout(int dim, int nbins)
@@ -67,6 +68,8 @@ Layout make_layout(int dim, int nbins)
     L.result = o;     o = align_up(o + 64, 256);
     L.flags = o;      o = align_up(o + kMaxDim * 4, 256);
     L.status = o;     o = align_up(o + 4, 256);
+    L.dev_iter = o;   o = align_up(o + 4, 256);                    // iteration counter of CUDA-graph replays
+    L.ring = o;       o = align_up(o + static_cast<size_t>(kRing) * 16, 256);   // their (I, sigma) log
     L.total = o;
     return L;
 }
@@ -202,9 +205,16 @@ struct vegas_ctx {
     size_t smem_bytes;
     double* h_result;        // pinned: result[8] then hist[dim*nbins]
     int* h_status;           // pinned
+    double* h_ring;          // pinned: kRing (I, sigma) pairs read back from graph replays
+    cudaEvent_t run_ev0, run_ev1;    // bracket a whole graph-replayed run
+    cudaStream_t gstream;            // internal capturable stream the graph is captured on and replayed in
+                                     // (the caller's stream may be the legacy default stream, which cannot capture)
     cudaEvent_t evA[kEvPool], evB[kEvPool];   // pair (n % kEvPool) brackets the n-th enqueued iteration
     uint64_t n_enqueued;             // iterations enqueued so far
     int refine_pending;              // refinements enqueued and not yet collected
+    int use_graph;                   // vegas_run_integration replays a captured step (vegas_use_cuda_graph)
+    cudaGraphExec_t gexec;           // captured {memset, launches, finalize, refine, commit} for the key below
+    uint64_t g_n, g_epl, g_seed; double g_alpha; int g_threads, g_ctas, g_rshift; const Instance* g_inst;
     cudaStream_t lane[kLanes];       // non-blocking streams: small launches of one iteration overlap on the GPU
     cudaEvent_t lane_done[kLanes], fork;
     uint64_t last_n;
@@ -310,6 +320,7 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
     a.e_hi = static_cast<uint32_t>(first >> 32);
     a.count = count;
     a.iteration = c->iteration;
+    a.iter_ptr = nullptr;
     const uint32_t k0 = static_cast<uint32_t>(seed), k1 = static_cast<uint32_t>(seed >> 32);
     for (int r = 0; r < 10; ++r) {
         a.rk0[r] = k0 + static_cast<uint32_t>(r) * 0x9E3779B9u;
@@ -393,7 +404,7 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->ws = static_cast<unsigned char*>(dev_workspace);
     c->L = L;
     c->iteration = 0; c->have_hist = false; c->have_sums = false;
-    c->h_result = nullptr; c->h_status = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0;
+    c->h_result = nullptr; c->h_status = nullptr; c->h_ring = nullptr; c->run_ev0 = nullptr; c->run_ev1 = nullptr; c->gstream = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0; c->use_graph = 1; c->gexec = nullptr;
     for (int i = 0; i < kEvPool; ++i) { c->evA[i] = nullptr; c->evB[i] = nullptr; }
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0;
@@ -413,6 +424,9 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->sm_clock_khz = khz;
     if (cudaHostAlloc(reinterpret_cast<void**>(&c->h_result), (8 + static_cast<size_t>(dim) * nbins) * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc(reinterpret_cast<void**>(&c->h_ring), kRing * 16, cudaHostAllocDefault) != cudaSuccess ||
+        cudaEventCreate(&c->run_ev0) != cudaSuccess || cudaEventCreate(&c->run_ev1) != cudaSuccess ||
+        cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess ||
         !create_event_pool(c) ||
         cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) != cudaSuccess || !create_lanes(c))
         return cleanup(fail(VEGAS_ECUDA, "pinned host buffer / event creation failed: %s", cudaGetErrorString(cudaGetLastError())));
@@ -433,10 +447,15 @@ void vegas_destroy(vegas_ctx* c)
     if (!c) return;
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_status) cudaFreeHost(c->h_status);
+    if (c->h_ring) cudaFreeHost(c->h_ring);
+    if (c->run_ev0) cudaEventDestroy(c->run_ev0);
+    if (c->run_ev1) cudaEventDestroy(c->run_ev1);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     for (int i = 0; i < kEvPool; ++i) {
         if (c->evA[i]) cudaEventDestroy(c->evA[i]);
         if (c->evB[i]) cudaEventDestroy(c->evB[i]);
     }
+    if (c->gexec) cudaGraphExecDestroy(c->gexec);
     if (c->fork) cudaEventDestroy(c->fork);
     for (int i = 0; i < kLanes; ++i) {
         if (c->lane[i]) cudaStreamDestroy(c->lane[i]);
@@ -481,8 +500,20 @@ int vegas_device_info(const vegas_ctx* c, int* sm_count, int* sm_clock_khz)
     return VEGAS_OK;
 }
 
+static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
+                             int* n_kernel_launches, bool graph_mode);
+
 int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
                           int* n_kernel_launches)
+{
+    return enqueue_iteration(c, n_events, events_per_launch, seed, n_kernel_launches, false);
+}
+
+// graph_mode: called between cudaStreamBeginCapture / EndCapture.  The iteration counter is read from device
+// memory (finalize advances it and logs (I, sigma) to the ring), no timing events are recorded, and the host-side
+// bookkeeping (iteration counter, event pool) is left to the caller.
+static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
+                             int* n_kernel_launches, bool graph_mode)
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (n_events < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
@@ -490,10 +521,11 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
     if (n_events > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
     const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
     const int evi = static_cast<int>(c->n_enqueued % kEvPool);
-    CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
+    if (!graph_mode) CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
     CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
     IterArgs a;
     fill_args(c, seed, 0, 0, a);
+    if (graph_mode) a.iter_ptr = reinterpret_cast<const uint32_t*>(c->ws + c->L.dev_iter);
     const int max_grid = c->ctas_per_sm * c->sm_count;
     // Launches of one iteration are independent (global event index; the histogram and the pass counter are
     // accumulated with global reductions; each lane has its own slot region), so when an iteration is cut into
@@ -532,8 +564,14 @@ int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_l
     }
     finalize_kernel<<<1, 32, 0, c->stream>>>(slots0, lanes, kLaneSlots, used_grid,
                                              reinterpret_cast<const unsigned long long*>(c->ws + c->L.npass),
-                                             n_events, reinterpret_cast<double*>(c->ws + c->L.result));
+                                             n_events, reinterpret_cast<double*>(c->ws + c->L.result),
+                                             graph_mode ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr,
+                                             graph_mode ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr, kRing);
     CUDA_TRY(cudaGetLastError());
+    if (n_kernel_launches) *n_kernel_launches = launches + 1;
+    c->have_hist = true;
+    c->last_launches = launches + 1;
+    if (graph_mode) return VEGAS_OK;
     CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
     c->n_enqueued += 1;
     c->iteration += 1;
@@ -713,6 +751,94 @@ int vegas_combine_iterations(int n, const double* I, const double* sg, double* m
     return VEGAS_OK;
 }
 
+// Capture one whole step {memset, iterate launches, finalize, refine, commit} of (n_events, epl, seed, alpha) with
+// the current launch shape into a CUDA graph (kept until the key changes).  In the captured step the iteration
+// counter lives in device memory: finalize logs (I, sigma) to a ring and advances it.
+static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha)
+{
+    if (c->gexec && c->g_n == n_events && c->g_epl == epl && c->g_seed == seed && c->g_alpha == alpha &&
+        c->g_threads == c->threads && c->g_ctas == c->ctas_per_sm && c->g_rshift == c->rshift && c->g_inst == c->inst)
+        return VEGAS_OK;
+    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+    CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
+    int rc = enqueue_iteration(c, n_events, epl, seed, nullptr, true);
+    if (rc == VEGAS_OK) rc = vegas_refine_enqueue(c, alpha);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);     // always leave capture mode
+    c->refine_pending = 0;
+    if (rc != VEGAS_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(VEGAS_ECUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    const cudaError_t e2 = cudaGraphInstantiate(&c->gexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { c->gexec = nullptr; return fail(VEGAS_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    c->g_n = n_events; c->g_epl = epl; c->g_seed = seed; c->g_alpha = alpha;
+    c->g_threads = c->threads; c->g_ctas = c->ctas_per_sm; c->g_rshift = c->rshift; c->g_inst = c->inst;
+    return VEGAS_OK;
+}
+
+// `total` replays of the captured step; (I, sigma) of every iteration into I[], sg[]; average device time per
+// iteration into *avg_ms.  One host synchronisation per kRing iterations.
+static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
+                              double* I, double* sg, double* avg_ms);
+
+static int run_steps_graph(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
+                           double* I, double* sg, double* avg_ms)
+{
+    int rc = vegas_refine_collect(c);
+    if (rc != VEGAS_OK && rc != VEGAS_EGRID) return rc;
+    // fork the internal stream from the caller's, run there, join back: stream order is kept for the caller
+    cudaStream_t user = c->stream;
+    CUDA_TRY(cudaEventRecord(c->fork, user));
+    CUDA_TRY(cudaStreamWaitEvent(c->gstream, c->fork, 0));
+    c->stream = c->gstream;
+    rc = run_steps_graph_on(c, total, n_events, epl, seed, alpha, I, sg, avg_ms);
+    c->stream = user;
+    if (cudaEventRecord(c->fork, c->gstream) == cudaSuccess) cudaStreamWaitEvent(user, c->fork, 0);
+    return rc;
+}
+
+static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
+                              double* I, double* sg, double* avg_ms)
+{
+    int rc;
+    rc = ensure_step_graph(c, n_events, epl, seed, alpha);
+    if (rc != VEGAS_OK) return rc;
+    uint32_t* h_it = reinterpret_cast<uint32_t*>(c->h_status) + 4;
+    *h_it = c->iteration;
+    CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.dev_iter, h_it, 4, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaEventRecord(c->run_ev0, c->stream));
+    for (int done = 0; done < total;) {
+        const int chunk = (total - done < kRing) ? total - done : kRing;
+        for (int i = 0; i < chunk; ++i) CUDA_TRY(cudaGraphLaunch(c->gexec, c->stream));
+        if (done + chunk == total) CUDA_TRY(cudaEventRecord(c->run_ev1, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(c->h_ring, c->ws + c->L.ring, kRing * 16, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaStreamSynchronize(c->stream));
+        for (int i = 0; i < chunk; ++i) {
+            const uint32_t it = c->iteration + static_cast<uint32_t>(done + i);
+            I[done + i] = c->h_ring[2 * (it % kRing) + 0];
+            sg[done + i] = c->h_ring[2 * (it % kRing) + 1];
+        }
+        done += chunk;
+    }
+    float ms = 0.f;
+    CUDA_TRY(cudaEventElapsedTime(&ms, c->run_ev0, c->run_ev1));
+    if (avg_ms) *avg_ms = static_cast<double>(ms) / total;
+    c->iteration += static_cast<uint32_t>(total);
+    c->have_hist = false;                                // the last step refined
+    c->have_sums = true;
+    c->last_n = n_events;
+    c->refine_pending = total;
+    rc = vegas_refine_collect(c);
+    return rc == VEGAS_EGRID ? VEGAS_OK : rc;            // a rejected refinement left its grid unchanged; the run went on
+}
+
+int vegas_use_cuda_graph(vegas_ctx* c, int enable)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    c->use_graph = enable ? 1 : 0;
+    return VEGAS_OK;
+}
+
 int vegas_run_integration(vegas_ctx* c, int n_iter, int n_warmup, uint64_t n_events, uint64_t events_per_launch,
                           uint64_t seed, double alpha, double* mean, double* error, double* chi2_dof,
                           double* iter_integral, double* iter_error, double* iter_kernel_ms)
@@ -725,6 +851,12 @@ int vegas_run_integration(vegas_ctx* c, int n_iter, int n_warmup, uint64_t n_eve
     if (!I) return fail(VEGAS_ENOMEM, "host allocation failed");
     double* sg = I + total;
     int rc = VEGAS_OK;
+    if (c->use_graph) {
+        if (n_events < 2 || events_per_launch == 0) { std::free(I); return fail(VEGAS_EINVAL, "n_events >= 2 and events_per_launch > 0 required"); }
+        double avg = 0.0;
+        rc = run_steps_graph(c, total, n_events, events_per_launch, seed, alpha, I, sg, &avg);
+        if (rc == VEGAS_OK && iter_kernel_ms) for (int it = 0; it < total; ++it) iter_kernel_ms[it] = avg;
+    } else
     for (int it = 0; it < total && rc == VEGAS_OK; ++it) {
         rc = vegas_iterate(c, n_events, events_per_launch, seed, &I[it], &sg[it], nullptr);
         if (rc != VEGAS_OK) break;

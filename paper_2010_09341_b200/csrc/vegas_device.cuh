@@ -35,7 +35,8 @@ struct IterArgs {
     uint32_t e_lo_first;   // low word of the first global event index of this launch
     uint32_t e_hi;         // high word (uniform within a launch: launches never straddle 2^32)
     uint32_t count;        // events in this launch (<= 2^31)
-    uint32_t iteration;    // Philox counter word 2
+    uint32_t iteration;    // Philox counter word 2 (used when iter_ptr is NULL)
+    const uint32_t* iter_ptr;  // device: the counter lives in memory (CUDA-graph replays of run_integration)
     uint32_t rk0[10], rk1[10];  // Philox round keys: k + r * Weyl
     int dim, nbins;
     int rshift;            // log2 of the number R of lane-indexed histogram replicas in shared memory
@@ -275,8 +276,8 @@ struct U32 : F {
 // event_front: S1 + S2 + the per-coordinate part of S3.  Leaves the integrand's accumulated state in
 // `integrand` and returns J.
 template <class F, int D, int NB, int TSTRIDE, class BinSink>
-__device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
-                                                        BinSink&& sink, F& integrand)
+__device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint32_t it, uint32_t e_lo, const void* tab_,
+                                                        int toff, BinSink&& sink, F& integrand)
 {
     using real = typename F::real;
     constexpr bool kF64 = (sizeof(real) == 8);
@@ -293,11 +294,11 @@ __device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint3
             if (!D && k >= d) break;
             int i; double frac;
             if constexpr (F::kU32) {                     // one 32-bit word per coordinate, four per Philox block
-                if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 2), a, r);
+                if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 2), a, r);
                 const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
                 bin_frac64_u32(w, N, i, frac);
             } else {                                     // 52 bits of two words per coordinate
-                if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 1), a, r);
+                if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 1), a, r);
                 const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
                 bin_frac64(w_lo, w_hi, N, i, frac);
             }
@@ -314,7 +315,7 @@ __device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint3
 #pragma unroll
         for (int k = 0; k < (D ? D : kMaxDim); ++k) {
             if (!D && k >= d) break;
-            if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, a.iteration, static_cast<uint32_t>(k >> 2), a, r);
+            if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 2), a, r);
             const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
             int i; float frac;
             bin_frac32(w, N, i, frac);
@@ -337,7 +338,7 @@ __device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo
 {
     using real = typename F::real;
     F integrand;
-    const real J = event_front<F, D, NB, TSTRIDE>(a, e_lo, tab_, toff, sink, integrand);
+    const real J = event_front<F, D, NB, TSTRIDE>(a, a.iteration, e_lo, tab_, toff, sink, integrand);
     pass = integrand.precheck(a.ic);
     const real f = pass ? integrand.end(a.ic, D ? D : a.dim) : real(0);
     J_out = J;

@@ -152,6 +152,7 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
+    const uint32_t it = a.iter_ptr ? *a.iter_ptr : a.iteration;   // S1 counter word 2
     for (int i = tid; i < cells * R; i += blockDim.x) sh_hist[i] = 0.0;
     {
         const real2* gt = static_cast<const real2*>(a.table);
@@ -190,7 +191,7 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
             BinPack<D> bp;
             bp.clear();
             F integrand;
-            const real J = event_front<F, D, NB, TREP>(a, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
+            const real J = event_front<F, D, NB, TREP>(a, it, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
                                                        [&](int k, int i, real) { bp.set(k, i); }, integrand);
             accumulate(J, integrand.end(a.ic, d), bp);
             np += 1u;
@@ -230,7 +231,7 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
             real J = real(0);
             if (idx < a.count) {
                 bp.clear();
-                J = event_front<F, D, NB, TREP>(a, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
+                J = event_front<F, D, NB, TREP>(a, it, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
                                                 [&](int k, int i, real) { bp.set(k, i); }, integrand);
                 pass = integrand.precheck(a.ic);
             }
@@ -305,7 +306,8 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 __global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__ slots, int nlanes, int lane_stride,
                                                       int per_lane,
                                                       const unsigned long long* __restrict__ npass,
-                                                      unsigned long long n_events, double* __restrict__ result)
+                                                      unsigned long long n_events, double* __restrict__ result,
+                                                      uint32_t* dev_iter, double* __restrict__ ring, int ring_len)
 {
     const int lane = threadIdx.x;
     Comp t1{0.0, 0.0}, t2{0.0, 0.0};
@@ -327,6 +329,12 @@ __global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__
         result[3] = S2;
         result[4] = static_cast<double>(*npass);
         result[5] = n;
+        if (ring) {                                      // graph replays: log (I, sigma) and advance the counter
+            const uint32_t it = *dev_iter;
+            ring[2 * (it % ring_len) + 0] = I;
+            ring[2 * (it % ring_len) + 1] = result[1];
+            *dev_iter = it + 1u;
+        }
     }
 }
 

@@ -47,6 +47,7 @@ SIGNATURES = {
     "vegas_run_integration": (C.c_int, [_vp, C.c_int, C.c_int, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, _dp, _dp,
                                         _dp, _dp, _dp, _dp]),
     "vegas_tune_events_per_launch": (C.c_int, [_vp, C.c_uint64, C.c_uint64, _u64p, C.c_int, _u64p, _dp]),
+    "vegas_use_cuda_graph": (C.c_int, [_vp, C.c_int]),
     "vegas_combine_iterations": (C.c_int, [C.c_int, _dp, _dp, _dp, _dp, _dp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
@@ -145,6 +146,9 @@ class Vegas:
                                          C.byref(m), C.byref(e), C.byref(c2), _d(I), _d(s), _d(ms)),
              "vegas_run_integration")
         return m.value, e.value, c2.value, dict(integral=I, error=s, kernel_ms=ms)
+
+    def use_cuda_graph(self, enable=True):
+        _chk(lib().vegas_use_cuda_graph(self._h, 1 if enable else 0), "vegas_use_cuda_graph")
 
     def tune_events_per_launch(self, n_events, candidates, seed=0):
         """The batch-size study of PAPER.md:L57-L65 on this GPU: (best candidate, {candidate: ms})."""
