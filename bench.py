@@ -306,7 +306,16 @@ def run_b200(args):
         if not args.no_cpu_baseline and world == 1:
             ns = min(n, args.cpu_sample)
             cdt, cores = oracle_steps(w, ns, 1, 0)
+            n1 = min(ns, 5 * 10**6)
+            from oracle import oracle as _O
+            o1 = _O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+            t1 = time.perf_counter()
+            o1.iterate(n1, w.seed, threads=1)
+            o1.refine(w.alpha)
+            t1 = time.perf_counter() - t1
             out["cpu_baseline"] = {"value": ns / cdt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                   "single_thread": {"value": n1 / t1, "unit": UNIT, "cores": 1,
+                                                     "sample": "one step over the first %d events, plain single-threaded C loop" % n1},
                                    "sample": "one step (iterate + refine) over the first %d of %d events of the same "
                                              "workload, oracle/vegas_oracle.c on %d threads" % (ns, n, cores)}
         print(json.dumps(out))

@@ -27,7 +27,8 @@ def run_config(name, w, n_iter=None, epl=0, tune=False):
         cands = [c for c in (10**4, 10**5, 10**6, 10**7, 10**8) if c <= w.n_events]
         tuned = g.tune_events_per_launch(w.n_events, cands, seed=w.seed)
     g.reset()
-    ms, wall, res, passf = [], [], [], []
+    import torch
+    ms, wall, res, passf, rms = [], [], [], [], []
     for _ in range(n_iter):
         t0 = time.perf_counter()
         I, s, _ = g.iterate(w.n_events, epl, w.seed, want_hist=False)
@@ -35,12 +36,17 @@ def run_config(name, w, n_iter=None, epl=0, tune=False):
         ms.append(g.last_sums()[2])
         passf.append(g.last_npass() / w.n_events)
         res.append((I, s))
-        g.refine(w.alpha)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.refine_enqueue(w.alpha)
+        e1.record()
+        g.refine_collect()
+        rms.append(e0.elapsed_time(e1))     # refine_kernel + refine_commit_kernel on the current stream
     out = {"config": name, "workload": w.name, "n_events": w.n_events, "events_per_launch": epl or w.n_events,
            "iterations": n_iter, "kernel_ms_median": statistics.median(ms), "kernel_ms_best": min(ms),
            "events_per_s_median": w.n_events / (statistics.median(ms) * 1e-3),
            "events_per_s_best": w.n_events / (min(ms) * 1e-3),
-           "wall_ms_median": statistics.median(wall), "launch_shape": g.launch_shape(),
+           "wall_ms_median": statistics.median(wall), "refine_ms_median": statistics.median(rms), "launch_shape": g.launch_shape(),
            "pass_fraction_first_last": [passf[0], passf[-1]], "last_result": res[-1],
            "tuned_events_per_launch": tuned[0] if tuned else None, "tune_ms": tuned[1] if tuned else None}
     g.close()
