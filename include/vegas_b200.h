@@ -63,7 +63,8 @@ enum { VEGAS_FP64 = 0, VEGAS_FP32_EVAL = 1,
  *   3 lo_2to2        {sqrt_s, sqrt_shat_min, cos_cut, pdf_a, pdf_b=5}   synthetic LO 2->2, dim = 3          configs[4]
  *   4 toy_sum        {}                                  f = sum_k x_k
  */
-enum { VEGAS_GAUSS_SYM = 0, VEGAS_GAUSS_DOUBLE = 1, VEGAS_GENZ_OSC_PEAK = 2, VEGAS_LO_2TO2 = 3, VEGAS_TOY_SUM = 4 };
+enum { VEGAS_GAUSS_SYM = 0, VEGAS_GAUSS_DOUBLE = 1, VEGAS_GENZ_OSC_PEAK = 2, VEGAS_LO_2TO2 = 3, VEGAS_TOY_SUM = 4,
+       VEGAS_USER = 5 /* run-time compiled user integrand: vegas_create_custom only */ };
 
 /* Device bytes the caller must provide to vegas_create for this (dim, nbins).  0 if out of range. */
 size_t vegas_workspace_bytes(int dim, int nbins);
@@ -76,6 +77,21 @@ size_t vegas_workspace_bytes(int dim, int nbins);
  * (workspace_bytes too small), VEGAS_EUNSUPPORTED (no instance), VEGAS_ECUDA. */
 int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
                  int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* User integrand, compiled at run time (the paper's `integrator.compile(integrand)`: the user
+ * writes a function of the points in the unit hypercube).  `source` is a NUL-terminated
+ * translation unit in the subset of C that is also valid CUDA device code and must define
+ *     VEGAS_INTEGRAND double vegas_user_integrand(const double* x, int dim, const double* params)
+ * (VEGAS_INTEGRAND expands to __device__ here; helper functions need the same prefix).  NVRTC compiles it for
+ * sm_100a together with the library's own kernel templates (the headers next to the library, csrc/), without
+ * fused-multiply-add contraction of the user's arithmetic, into the same iterate kernel the built-in integrands
+ * use (run-time shaped: any dim <= 32, any nbins, fp64); everything else (grid, refine, run_integration, parity
+ * hook) works as for vegas_create.  params (0..16 doubles) are copied.  precision: VEGAS_FP64 or VEGAS_FP64_U32.
+ * On a compilation error the compiler log is available from vegas_last_error().
+ * Errors: VEGAS_EINVAL (NULL source, ranges, > 16 params, precision), VEGAS_EUNSUPPORTED (NVRTC compilation
+ * failed), VEGAS_ENOMEM, VEGAS_ECUDA. */
+int vegas_create_custom(vegas_ctx** out, int dim, int nbins, const char* source, const double* params, int n_params,
+                        int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
 
 /* One Vegas iteration (S1-S6): n_events events, global event index e in [0, n_events), cut into
  * ceil(n_events/events_per_launch) kernel launches (PAPER.md:L57-L65 `events_limit`; results do not

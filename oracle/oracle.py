@@ -76,6 +76,7 @@ def lib():
         L.oracle_get_table.argtypes = [vp, dp, dp, dp]
         L.oracle_get_gauss_consts.argtypes = [vp, dp]
         L.oracle_combine.argtypes = [C.c_int, dp, dp, dp, dp, dp]
+        L.oracle_set_user_integrand.argtypes = [vp, vp]
         _lib = L
     return _lib
 
@@ -124,6 +125,29 @@ class Oracle:
             raise OracleError(rc, "create")
         self.dim, self.nbins, self.integrand_id, self.precision = dim, nbins, integrand_id, precision
         self.npass = None
+
+    @classmethod
+    def custom(cls, dim, nbins, c_source, params=(), precision=FP64):
+        """ID_USER: compiles `c_source` (plain C defining vegas_user_integrand(x, dim, params); the prefix macro
+        VEGAS_INTEGRAND expands to nothing) with gcc -O2 -ffp-contract=off and plugs it into S3."""
+        import hashlib
+        import tempfile
+        tag = hashlib.sha1(c_source.encode()).hexdigest()[:16]
+        d = os.path.join(tempfile.gettempdir(), "vegas_oracle_user")
+        os.makedirs(d, exist_ok=True)
+        so = os.path.join(d, "user_%s.so" % tag)
+        if not os.path.exists(so):
+            src = os.path.join(d, "user_%s.c" % tag)
+            with open(src, "w") as f:
+                f.write("#include <math.h>\n#define VEGAS_INTEGRAND\n" + c_source + "\n")
+            subprocess.run(["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared", src,
+                            "-o", so + ".tmp", "-lm"], check=True)
+            os.replace(so + ".tmp", so)
+        ulib = C.CDLL(so)
+        self = cls(dim, nbins, 5, params, precision)
+        self._user_lib = ulib                                  # keep the code mapped
+        _chk(lib().oracle_set_user_integrand(self._h, C.cast(ulib.vegas_user_integrand, C.c_void_p)), "set_user")
+        return self
 
     def close(self):
         if getattr(self, "_h", None):

@@ -44,7 +44,10 @@ enum { ORACLE_FP64 = 0, ORACLE_FP32_EVAL = 1, ORACLE_FP64_U32 = 2 };
  * DESIGN.md reading R3.  is_f64() is true for both fp64 modes. */
 #define is_f64(c) ((c)->precision != ORACLE_FP32_EVAL)
 #define ubits(c) ((c)->precision == ORACLE_FP64 ? 52 : ((c)->precision == ORACLE_FP64_U32 ? 32 : 23))
-enum { ID_GAUSS_SYM = 0, ID_GAUSS_DOUBLE = 1, ID_GENZ_OSC_PEAK = 2, ID_LO_2TO2 = 3, ID_TOY_SUM = 4 };
+enum { ID_GAUSS_SYM = 0, ID_GAUSS_DOUBLE = 1, ID_GENZ_OSC_PEAK = 2, ID_LO_2TO2 = 3, ID_TOY_SUM = 4, ID_USER = 5 };
+/* ID_USER: a user-supplied integrand f(x, dim, params) (the user writes the function of the
+ * points); the tests compile the same C source with gcc that the CUDA side compiles at run time. */
+typedef double (*oracle_user_fn)(const double *x, int dim, const double *params);
 
 /* fl64(pi) = 3.141592653589793115997963... */
 #define ORACLE_PI 0x1.921fb54442d18p+1
@@ -57,6 +60,7 @@ typedef struct oracle_ctx {
     int n_params;
     double params[ORACLE_MAX_PARAMS];
     uint32_t iteration;   /* counter word 2 of S1; +1 per committed iteration */
+    oracle_user_fn user_fn;   /* ID_USER: set by oracle_set_user_integrand before the first event */
     int uniform;          /* 1 after create/reset: table uses wd=fl(1/N) (S2, reading R6) */
     int have_hist;
     double *edges;        /* [dim][nbins+1] fp64 master edges E */
@@ -246,6 +250,9 @@ static int setup_integrand(oracle_ctx *c)
     case ID_TOY_SUM:
         if (c->n_params != 0) return ORACLE_EINVAL;
         return ORACLE_OK;
+    case ID_USER:             /* params are handed to the user function as they are */
+        if (!is_f64(c) || c->n_params > 16) return ORACLE_EINVAL;
+        return ORACLE_OK;
     default:
         return ORACLE_EUNSUPPORTED;
     }
@@ -376,6 +383,8 @@ static double eval_fp64(const oracle_ctx *c, const double *x, int *pass_out)
         for (int k = 0; k < d; ++k) f = f + x[k];
         return f;
     }
+    case ID_USER:
+        return c->user_fn ? c->user_fn(x, d, c->params) : NAN;
     default:
         return NAN;
     }
@@ -400,6 +409,8 @@ static float eval_fp32(const oracle_ctx *c, const float *x)
         for (int k = 0; k < d; ++k) f = f + x[k];
         return f;
     }
+    case ID_USER:
+        return c->user_fn ? c->user_fn(x, d, c->params) : NAN;
     default:
         return NAN;
     }
@@ -712,5 +723,13 @@ int oracle_combine(int n, const double *I, const double *sigma, double *mean, do
     *mean = (double)m;
     *err = (double)(1.0L / sqrtl(sum_w));
     if (chi2_dof) *chi2_dof = (n > 1) ? (double)(chi2 / (n - 1)) : 0.0;
+    return ORACLE_OK;
+}
+
+/* ID_USER: the function evaluated in S3. */
+int oracle_set_user_integrand(oracle_ctx *c, oracle_user_fn fn)
+{
+    if (!c || !fn || c->integrand_id != ID_USER) return ORACLE_EINVAL;
+    c->user_fn = fn;
     return ORACLE_OK;
 }

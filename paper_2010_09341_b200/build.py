@@ -15,8 +15,9 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libvegas_b200.so")
-SOURCES = [os.path.join(CSRC, "vegas_api.cu"), os.path.join(CSRC, "pipe_bench.cu")]
+SOURCES = [os.path.join(CSRC, "vegas_api.cu"), os.path.join(CSRC, "pipe_bench.cu"), os.path.join(CSRC, "vegas_rtc.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "vegas_kernels.cuh"), os.path.join(CSRC, "vegas_device.cuh"),
+                  os.path.join(CSRC, "vegas_user.cuh"), os.path.join(CSRC, "vegas_rtc.h"),
                   os.path.join(INCLUDE, "vegas_b200.h")]
 
 NVCC_FLAGS = [
@@ -26,6 +27,7 @@ NVCC_FLAGS = [
     # the host-side constant setup must not be contracted either
     "-Xcompiler", "-fPIC,-ffp-contract=off",
     "-shared",
+    "-lnvrtc",                                       # run-time compilation of user integrands (vegas_create_custom)
 ]
 
 

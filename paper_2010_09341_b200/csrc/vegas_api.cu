@@ -15,6 +15,7 @@
 
 #include "../../include/vegas_b200.h"
 #include "vegas_kernels.cuh"
+#include "vegas_rtc.h"
 
 namespace {
 
@@ -27,7 +28,7 @@ constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the i
 constexpr int kMaxSlots = kLanes * kLaneSlots;
 constexpr double kPi = 0x1.921fb54442d18p+1;   // fl64(pi)
 
-thread_local char g_err[512] = "";
+thread_local char g_err[4096] = "";
 
 int fail(int code, const char* fmt, ...)
 {
@@ -90,7 +91,34 @@ struct Instance {
     DebugFn debug;
     AttrFn set_smem;
     OccFn occupancy;
+    const void* rt_iterate;          // run-time compiled instance (vegas_create_custom): cudaKernel_t handles used
+    const void* rt_debug;            // instead of the four function pointers above
 };
+
+// One interface for compiled-in and run-time compiled instances.
+cudaError_t inst_launch(const Instance* in, const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    if (!in->rt_iterate) return in->launch(a, grid, threads, smem, st);
+    void* args[] = {const_cast<IterArgs*>(&a)};
+    return cudaLaunchKernel(in->rt_iterate, dim3(grid), dim3(threads), args, smem, st);
+}
+cudaError_t inst_debug(const Instance* in, const IterArgs& a, int grid, int threads, cudaStream_t st, int32_t* bins,
+                       double* x, double* jac, double* f, double* wf, int32_t* pass)
+{
+    if (!in->rt_debug) return in->debug(a, grid, threads, st, bins, x, jac, f, wf, pass);
+    void* args[] = {const_cast<IterArgs*>(&a), &bins, &x, &jac, &f, &wf, &pass};
+    return cudaLaunchKernel(in->rt_debug, dim3(grid), dim3(threads), args, 0, st);
+}
+cudaError_t inst_set_smem(const Instance* in, int smem_bytes)
+{
+    if (!in->rt_iterate) return in->set_smem(smem_bytes);
+    return cudaFuncSetAttribute(in->rt_iterate, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+}
+cudaError_t inst_occupancy(const Instance* in, int* ctas, int threads, size_t smem)
+{
+    if (!in->rt_iterate) return in->occupancy(ctas, threads, smem);
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, in->rt_iterate, threads, smem);
+}
 
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t launch_iterate(const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
@@ -129,11 +157,11 @@ constexpr int queue_entry_bytes()
 #define VEGAS_TUNED(ID, F, D, NB, RS, TREP, HB, PREC, MAXT, CTAS, THREADS)                               \
     Instance { ID, D, NB, PREC, RS, TREP, MAXT, CTAS, THREADS, queue_entry_bytes<F, D>(), launch_iterate<F, D, NB, RS, TREP, HB, MAXT, 1>, \
                launch_debug<F, D>, set_smem_attr<F, D, NB, RS, TREP, HB, MAXT, 1>,                       \
-               query_occupancy<F, D, NB, RS, TREP, HB, MAXT, 1> }
+               query_occupancy<F, D, NB, RS, TREP, HB, MAXT, 1>, nullptr, nullptr }
 #define VEGAS_GENERIC(ID, F, D, PREC)                                                                    \
     Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, queue_entry_bytes<F, D>(), launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,          \
                launch_debug<F, D>, set_smem_attr<F, D, 0, -1, 1, 0, 1024, 1>,                            \
-               query_occupancy<F, D, 0, -1, 1, 0, 1024, 1> }
+               query_occupancy<F, D, 0, -1, 1, 0, 1024, 1>, nullptr, nullptr }
 
 const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GAUSS_SYM, GaussSym, 4, 50, 5, 8, 4, VEGAS_FP64, 1024, 1, 1024),            // configs[0]
@@ -183,6 +211,7 @@ int expected_params(int id, int dim)
         case VEGAS_GENZ_OSC_PEAK: return 1 + dim;
         case VEGAS_LO_2TO2: return 5;
         case VEGAS_TOY_SUM: return 0;
+        case VEGAS_USER: return -2;          // any count up to kMaxUserParams (checked by vegas_create_custom)
         default: return -1;
     }
 }
@@ -212,6 +241,9 @@ struct vegas_ctx {
     cudaEvent_t evA[kEvPool], evB[kEvPool];   // pair (n % kEvPool) brackets the n-th enqueued iteration
     uint64_t n_enqueued;             // iterations enqueued so far
     int refine_pending;              // refinements enqueued and not yet collected
+    cudaLibrary_t rt_lib;            // vegas_create_custom: the loaded cubin and its Instance (owned)
+    Instance* rt_inst;
+    int n_user_params;
     int use_graph;                   // vegas_run_integration replays a captured step (vegas_use_cuda_graph)
     cudaGraphExec_t gexec;           // captured {memset, launches, finalize, refine, commit} for the key below
     uint64_t g_n, g_epl, g_seed; double g_alpha; int g_threads, g_ctas, g_rshift; const Instance* g_inst;
@@ -262,6 +294,9 @@ int setup_integrand(vegas_ctx* c, const double* p)
             c->ic.ha = p[3];
             return VEGAS_OK;
         }
+        case VEGAS_USER:
+            for (int i = 0; i < c->n_user_params; ++i) c->ic.user_params[i] = p[i];
+            return VEGAS_OK;
         default: return VEGAS_OK;
     }
 }
@@ -299,9 +334,9 @@ int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
     if (rshift < 0 || rshift > 5) return fail(VEGAS_EINVAL, "histogram of %d x %d cells does not fit in shared memory with %d CTAs/SM", c->dim, c->nbins, ctas);
     const size_t smem = iterate_smem_bytes(c, in, rshift, threads);
     if (smem > static_cast<size_t>(c->smem_optin)) return fail(VEGAS_EINVAL, "needs %zu bytes of shared memory per CTA, device allows %d", smem, c->smem_optin);
-    CUDA_TRY(in->set_smem(static_cast<int>(smem)));
+    CUDA_TRY(inst_set_smem(in, static_cast<int>(smem)));
     int occ = 0;
-    CUDA_TRY(in->occupancy(&occ, threads, smem));
+    CUDA_TRY(inst_occupancy(in, &occ, threads, smem));
     if (occ < 1) return fail(VEGAS_EINVAL, "launch shape (%d threads, %zu B smem) cannot run", threads, smem);
     if (occ < ctas) ctas = occ;
     if (ctas * c->sm_count > kLaneSlots) ctas = kLaneSlots / c->sm_count;
@@ -371,8 +406,22 @@ size_t vegas_workspace_bytes(int dim, int nbins)
     return make_layout(dim, nbins).total;
 }
 
+static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
+                         int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream,
+                         const Instance* rt_inst);
+
 int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
                  int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (integrand_id == VEGAS_USER) return fail(VEGAS_EINVAL, "user integrands are created with vegas_create_custom");
+    return create_common(out, dim, nbins, integrand_id, params, n_params, precision, dev_workspace, workspace_bytes,
+                         cuda_stream, nullptr);
+}
+
+// rt_inst != NULL: a run-time compiled instance (vegas_create_custom) replaces the table lookup.
+static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
+                         int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream,
+                         const Instance* rt_inst)
 {
     if (!out) return fail(VEGAS_EINVAL, "out is NULL");
     *out = nullptr;
@@ -381,10 +430,11 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     const int max_bins = (precision == VEGAS_FP32_EVAL) ? 511 : 4095;     // m*N must be exact (S2)
     if (nbins < 2 || nbins > max_bins) return fail(VEGAS_EINVAL, "nbins %d not in 2..%d", nbins, max_bins);
     const int need = expected_params(integrand_id, dim);
-    if (need < 0) return fail(VEGAS_EUNSUPPORTED, "integrand_id %d unknown", integrand_id);
-    if (n_params != need || (need > 0 && !params)) return fail(VEGAS_EINVAL, "integrand %d with dim %d takes %d params, got %d", integrand_id, dim, need, n_params);
-    const Instance* tuned = find_tuned(integrand_id, dim, nbins, precision);
-    const Instance* inst = find_generic(integrand_id, dim, precision);
+    if (need == -1) return fail(VEGAS_EUNSUPPORTED, "integrand_id %d unknown", integrand_id);
+    if (need == -2) { if (n_params < 0 || n_params > kMaxUserParams || (n_params > 0 && !params)) return fail(VEGAS_EINVAL, "a user integrand takes 0..%d params", kMaxUserParams); }
+    else if (n_params != need || (need > 0 && !params)) return fail(VEGAS_EINVAL, "integrand %d with dim %d takes %d params, got %d", integrand_id, dim, need, n_params);
+    const Instance* tuned = rt_inst ? nullptr : find_tuned(integrand_id, dim, nbins, precision);
+    const Instance* inst = rt_inst ? rt_inst : find_generic(integrand_id, dim, precision);
     if (!inst) return fail(VEGAS_EUNSUPPORTED, "no compiled kernel for integrand %d, dim %d, precision %d", integrand_id, dim, precision);
     if (!dev_workspace) return fail(VEGAS_EINVAL, "dev_workspace is NULL");
     if (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) return fail(VEGAS_EINVAL, "dev_workspace must be 256-byte aligned");
@@ -407,7 +457,8 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     c->h_result = nullptr; c->h_status = nullptr; c->h_ring = nullptr; c->run_ev0 = nullptr; c->run_ev1 = nullptr; c->gstream = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0; c->use_graph = 1; c->gexec = nullptr;
     for (int i = 0; i < kEvPool; ++i) { c->evA[i] = nullptr; c->evB[i] = nullptr; }
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
-    c->last_n = 0; c->last_launches = 0;
+    c->last_n = 0; c->last_launches = 0; c->rt_lib = nullptr; c->rt_inst = nullptr;
+    c->n_user_params = n_params;
     int rc = setup_integrand(c, params);
     if (rc != VEGAS_OK) { delete c; return rc; }
 
@@ -442,6 +493,36 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
     return VEGAS_OK;
 }
 
+int vegas_create_custom(vegas_ctx** out, int dim, int nbins, const char* source, const double* params, int n_params,
+                        int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out) return fail(VEGAS_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (!source) return fail(VEGAS_EINVAL, "source is NULL");
+    if (dim < 1 || dim > kMaxDim) return fail(VEGAS_EINVAL, "dim %d not in 1..%d", dim, kMaxDim);
+    if (precision != VEGAS_FP64 && precision != VEGAS_FP64_U32) return fail(VEGAS_EINVAL, "user integrands are fp64: precision VEGAS_FP64 or VEGAS_FP64_U32");
+    if (n_params < 0 || n_params > kMaxUserParams || (n_params > 0 && !params)) return fail(VEGAS_EINVAL, "a user integrand takes 0..%d params", kMaxUserParams);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        (void)cudaGetLastError();
+        return fail(VEGAS_ECUDA, "no CUDA device (there is no CPU fallback)");
+    }
+    vegas_rtc_result r;
+    std::string log;
+    int rc = vegas_rtc_compile(dim, precision, source, &r, &log);
+    if (rc != VEGAS_OK) return fail(rc, "run-time compilation of the user integrand failed:\n%s", log.c_str());
+    Instance* in = new (std::nothrow) Instance{VEGAS_USER, dim, 0, precision, -1, 1, 1024, 2, 512, 0, nullptr, nullptr,
+                                               nullptr, nullptr, reinterpret_cast<const void*>(r.iterate),
+                                               reinterpret_cast<const void*>(r.debug)};
+    if (!in) { cudaLibraryUnload(r.library); return fail(VEGAS_ENOMEM, "host allocation failed"); }
+    rc = create_common(out, dim, nbins, VEGAS_USER, params, n_params, precision, dev_workspace, workspace_bytes,
+                       cuda_stream, in);
+    if (rc != VEGAS_OK) { delete in; cudaLibraryUnload(r.library); return rc; }
+    (*out)->rt_lib = r.library;
+    (*out)->rt_inst = in;
+    return VEGAS_OK;
+}
+
 void vegas_destroy(vegas_ctx* c)
 {
     if (!c) return;
@@ -456,6 +537,8 @@ void vegas_destroy(vegas_ctx* c)
         if (c->evB[i]) cudaEventDestroy(c->evB[i]);
     }
     if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->rt_lib) cudaLibraryUnload(c->rt_lib);
+    delete c->rt_inst;
     if (c->fork) cudaEventDestroy(c->fork);
     for (int i = 0; i < kLanes; ++i) {
         if (c->lane[i]) cudaStreamDestroy(c->lane[i]);
@@ -551,7 +634,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
         const int grid = want < static_cast<uint64_t>(max_grid) ? static_cast<int>(want) : max_grid;
         const int ln = launches % lanes;
         a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
-        CUDA_TRY(c->inst->launch(a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
+        CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
         if (grid > used_grid) used_grid = grid;
         done += cnt;
         ++launches;
@@ -945,7 +1028,7 @@ int vegas_debug_events(vegas_ctx* c, uint64_t first_event, uint32_t count, uint6
     int32_t* d_pass = reinterpret_cast<int32_t*>(tmp + b_bins + b_x + 3 * b_s);
     IterArgs a;
     fill_args(c, seed, first_event, count, a);
-    cudaError_t e = c->inst->debug(a, static_cast<int>((count + 127) / 128), 128, c->stream, d_bins, d_x, d_jac, d_f, d_wf, d_pass);
+    cudaError_t e = inst_debug(c->inst, a, static_cast<int>((count + 127) / 128), 128, c->stream, d_bins, d_x, d_jac, d_f, d_wf, d_pass);
     auto copy = [&](void* dst, const void* src, size_t n) {
         if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToHost, c->stream);
     };

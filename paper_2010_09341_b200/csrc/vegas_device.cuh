@@ -5,8 +5,20 @@
 // S4 weight.  Everything here stays in registers; the only memory touched is the (lo, wd) mapping table
 // in shared memory.  No code is shared with oracle/.
 #pragma once
+#ifdef __CUDACC_RTC__
+// run-time compilation of a user integrand (vegas_create_custom, NVRTC): no host headers
+typedef unsigned int uint32_t;
+typedef int int32_t;
+typedef unsigned long long uint64_t;
+namespace std {
+template <bool B, class T, class F> struct conditional { typedef T type; };
+template <class T, class F> struct conditional<false, T, F> { typedef F type; };
+}
+#else
 #include <cstdint>
+#include <type_traits>
 #include <cuda_runtime.h>
+#endif
 
 namespace vegas {
 
@@ -25,7 +37,11 @@ struct IntegrandConsts {
     float zphi;
     float zc[kMaxDim];
     float zw[kMaxDim];
+    // user integrand compiled at run time (vegas_create_custom): its parameters
+    double user_params[16];
 };
+
+constexpr int kMaxUserParams = 16;
 
 struct IterArgs {
     const void* table;     // device: (lo, wd) per cell, [dim][nbins], double2 (fp64) or float2 (fp32)

@@ -15,7 +15,7 @@ from . import build as _build
 
 OK, EINVAL, ECUDA, ENOMEM, ESTATE, EUNSUPPORTED, EGRID = 0, -1, -2, -3, -4, -5, -6
 FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
-GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM = 0, 1, 2, 3, 4
+GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM, USER = 0, 1, 2, 3, 4, 5
 
 _vp, _dp, _ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
 _i32p, _u32p, _u64p, _szp = C.POINTER(C.c_int32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_size_t)
@@ -24,6 +24,7 @@ _i32p, _u32p, _u64p, _szp = C.POINTER(C.c_int32), C.POINTER(C.c_uint32), C.POINT
 SIGNATURES = {
     "vegas_workspace_bytes": (C.c_size_t, [C.c_int, C.c_int]),
     "vegas_create": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
+    "vegas_create_custom": (C.c_int, [C.POINTER(_vp), C.c_int, C.c_int, C.c_char_p, _dp, C.c_int, C.c_int, _vp, C.c_size_t, _vp]),
     "vegas_iterate": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _dp, _dp, _dp]),
     "vegas_refine": (C.c_int, [_vp, C.c_double]),
     "vegas_refine_enqueue": (C.c_int, [_vp, C.c_double]),
@@ -91,7 +92,10 @@ def workspace_bytes(dim, nbins):
 class Vegas:
     """One integrator state on the GPU: VegasFlow(n_dim, ...) + compile(integrand) of PAPER.md:L77-L78."""
 
-    def __init__(self, dim, nbins, integrand_id, params=(), precision=FP64, stream=None, device="cuda:0"):
+    def __init__(self, dim, nbins, integrand_id, params=(), precision=FP64, stream=None, device="cuda:0", source=None):
+        """integrand_id: a built-in integrand, or USER with `source` = C source of
+        `VEGAS_INTEGRAND double vegas_user_integrand(const double* x, int dim, const double* params)`
+        (vegas_create_custom: compiled at run time, the paper's compile(integrand))."""
         import torch  # device memory and stream only
 
         L = lib()
@@ -110,8 +114,12 @@ class Vegas:
         ptr = (self._ws.data_ptr() + 255) & ~255
         self._stream = stream if stream is not None else torch.cuda.current_stream(self._dev)
         h = _vp()
-        _chk(L.vegas_create(C.byref(h), dim, nbins, integrand_id, _d(p) if p.size else None, int(p.size), precision,
-                            _vp(ptr), nbytes, _vp(self._stream.cuda_stream)), "vegas_create")
+        if source is not None:
+            _chk(L.vegas_create_custom(C.byref(h), dim, nbins, source.encode(), _d(p) if p.size else None, int(p.size),
+                                       precision, _vp(ptr), nbytes, _vp(self._stream.cuda_stream)), "vegas_create_custom")
+        else:
+            _chk(L.vegas_create(C.byref(h), dim, nbins, integrand_id, _d(p) if p.size else None, int(p.size), precision,
+                                _vp(ptr), nbytes, _vp(self._stream.cuda_stream)), "vegas_create")
         self._h = h
         self.dim, self.nbins, self.integrand_id, self.precision = dim, nbins, integrand_id, precision
 
