@@ -292,6 +292,7 @@ int setup_integrand(vegas_ctx* c, const double* p)
             c->ic.hL = std::log(tau);
             c->ic.hcut = p[2];
             c->ic.ha = p[3];
+            c->ic.hLLs = (c->ic.hL * c->ic.hL) / s;
             return VEGAS_OK;
         }
         case VEGAS_USER:
