@@ -165,10 +165,10 @@ constexpr int queue_entry_bytes()
 
 const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GAUSS_SYM, GaussSym, 4, 50, 5, 8, 4, VEGAS_FP64, 1024, 1, 1024),            // configs[0]
-    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, 50, 5, 8, 8, VEGAS_FP64, 1024, 1, 1024),      // configs[1], [2]
+    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, 50, 5, 8, 4, VEGAS_FP64, 768, 1, 768),      // configs[1], [2]
     VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 0, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
     VEGAS_TUNED(VEGAS_LO_2TO2, Lo2to2, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),                // configs[4]
-    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, U32<GaussDouble>, 8, 50, 5, 8, 8, VEGAS_FP64_U32, 1024, 1, 1024),   // configs[1] with 32-bit uniforms
+    VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, U32<GaussDouble>, 8, 50, 5, 8, 4, VEGAS_FP64_U32, 768, 1, 768),   // configs[1] with 32-bit uniforms
     VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL),
@@ -322,10 +322,12 @@ int pick_rshift(const vegas_ctx* c, const Instance* in, int ctas, int threads)
 }
 
 // ctas/threads <= 0: the instance's default.  rshift < 0: the tuned instance's fixed R if it can be used,
-// else the largest R that fits.  A shape the tuned instance cannot take (another R) runs on the generic one.
+// else the largest R that fits.  A shape the tuned instance cannot take (another R, more threads than it was compiled
+// for) runs on the generic one.
 int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
 {
-    const Instance* in = (c->tuned && (rshift < 0 || rshift == c->tuned->rs)) ? c->tuned : c->generic;
+    const Instance* in = (c->tuned && (rshift < 0 || rshift == c->tuned->rs) && threads <= c->tuned->max_threads)
+                             ? c->tuned : c->generic;
     if (ctas <= 0) ctas = in->def_ctas;
     if (threads <= 0) threads = in->def_threads;
     if (threads < 32 || threads > in->max_threads || (threads & 31)) return fail(VEGAS_EINVAL, "threads_per_cta %d not in 32..%d (multiple of 32)", threads, in->max_threads);
