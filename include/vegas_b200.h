@@ -64,7 +64,8 @@ enum { VEGAS_FP64 = 0, VEGAS_FP32_EVAL = 1,
  *   4 toy_sum        {}                                  f = sum_k x_k
  */
 enum { VEGAS_GAUSS_SYM = 0, VEGAS_GAUSS_DOUBLE = 1, VEGAS_GENZ_OSC_PEAK = 2, VEGAS_LO_2TO2 = 3, VEGAS_TOY_SUM = 4,
-       VEGAS_USER = 5 /* run-time compiled user integrand: vegas_create_custom only */ };
+       VEGAS_USER = 5 /* run-time compiled user integrand: vegas_create_custom only */,
+       VEGAS_LO_2TO2_TAB = 6 /* lo_2to2 with a tabulated PDF: params {sqrt_s, sqrt_shat_min, cos_cut} + vegas_set_table */ };
 
 /* Device bytes the caller must provide to vegas_create for this (dim, nbins).  0 if out of range. */
 size_t vegas_workspace_bytes(int dim, int nbins);
@@ -92,6 +93,14 @@ int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const do
  * failed), VEGAS_ENOMEM, VEGAS_ECUDA. */
 int vegas_create_custom(vegas_ctx** out, int dim, int nbins, const char* source, const double* params, int n_params,
                         int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* lo_2to2_tab (PDF interpolation is part of the integrand in the paper's
+ * workloads -- a synthetic table stands in for a PDF grid): the toy PDF g(x) of lo_2to2 is replaced by four-point
+ * Lagrange (cubic) interpolation of `values[0..n-1]`, knots uniform in ln x: values[j] = g(tau^(1 - j/(n-1))),
+ * tau = (sqrt_shat_min/sqrt_s)^2, so values[0] = g(tau), values[n-1] = g(1).  4 <= n <= 4096; copied into the
+ * workspace.  vegas_iterate fails with VEGAS_ESTATE until a table is set.
+ * Errors: VEGAS_EINVAL (NULL, n out of range, another integrand), VEGAS_ECUDA. */
+int vegas_set_table(vegas_ctx* ctx, const double* values, int n);
 
 /* One Vegas iteration (S1-S6): n_events events, global event index e in [0, n_events), cut into
  * ceil(n_events/events_per_launch) kernel launches (PAPER.md:L57-L65 `events_limit`; results do not

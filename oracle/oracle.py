@@ -77,6 +77,9 @@ def lib():
         L.oracle_get_gauss_consts.argtypes = [vp, dp]
         L.oracle_combine.argtypes = [C.c_int, dp, dp, dp, dp, dp]
         L.oracle_set_user_integrand.argtypes = [vp, vp]
+        L.oracle_set_table.argtypes = [vp, dp, C.c_int]
+        L.oracle_tab_interp.argtypes = [dp, C.c_int, C.c_double]
+        L.oracle_tab_interp.restype = C.c_double
         _lib = L
     return _lib
 
@@ -259,6 +262,11 @@ class Oracle:
     def refine(self, alpha):
         _chk(lib().oracle_refine(self._h, float(alpha)), "refine")
 
+    def set_table(self, values):
+        """ID_LO_2TO2_TAB: the tabulated PDF G_j = g(x_j), x_j = tau^(1 - j/(M-1))."""
+        v = np.ascontiguousarray(values, dtype=np.float64)
+        _chk(lib().oracle_set_table(self._h, _dp(v), int(v.size)), "set_table")
+
     def run_integration(self, n_iter, n_events, seed, alpha, n_warmup=0, threads=1):
         """(n_warmup + n_iter) x (iterate, refine); combination of the last n_iter (oracle_combine).
         A refine rejected for a non-monotone grid (EGRID) leaves the grid unchanged and the run goes on."""
@@ -281,3 +289,9 @@ def combine(integral, sigma):
     m, e, c2 = C.c_double(), C.c_double(), C.c_double()
     _chk(lib().oracle_combine(int(I.size), _dp(I), _dp(s), C.byref(m), C.byref(e), C.byref(c2)), "combine")
     return m.value, e.value, c2.value
+
+
+def tab_interp(values, v):
+    """The four-point Lagrange interpolation of oracle_set_table's table at v (scalar)."""
+    t = np.ascontiguousarray(values, dtype=np.float64)
+    return float(lib().oracle_tab_interp(_dp(t), int(t.size), float(v)))

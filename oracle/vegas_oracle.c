@@ -44,7 +44,7 @@ enum { ORACLE_FP64 = 0, ORACLE_FP32_EVAL = 1, ORACLE_FP64_U32 = 2 };
  * DESIGN.md reading R3.  is_f64() is true for both fp64 modes. */
 #define is_f64(c) ((c)->precision != ORACLE_FP32_EVAL)
 #define ubits(c) ((c)->precision == ORACLE_FP64 ? 52 : ((c)->precision == ORACLE_FP64_U32 ? 32 : 23))
-enum { ID_GAUSS_SYM = 0, ID_GAUSS_DOUBLE = 1, ID_GENZ_OSC_PEAK = 2, ID_LO_2TO2 = 3, ID_TOY_SUM = 4, ID_USER = 5 };
+enum { ID_GAUSS_SYM = 0, ID_GAUSS_DOUBLE = 1, ID_GENZ_OSC_PEAK = 2, ID_LO_2TO2 = 3, ID_TOY_SUM = 4, ID_USER = 5, ID_LO_2TO2_TAB = 6 };
 /* ID_USER: a user-supplied integrand f(x, dim, params) (the user writes the function of the
  * points); the tests compile the same C source with gcc that the CUDA side compiles at run time. */
 typedef double (*oracle_user_fn)(const double *x, int dim, const double *params);
@@ -60,6 +60,7 @@ typedef struct oracle_ctx {
     int n_params;
     double params[ORACLE_MAX_PARAMS];
     uint32_t iteration;   /* counter word 2 of S1; +1 per committed iteration */
+    double *tab; int ntab;    /* ID_LO_2TO2_TAB: tabulated PDF G_j = g(x_j), knots uniform in ln x (oracle_set_table) */
     oracle_user_fn user_fn;   /* ID_USER: set by oracle_set_user_integrand before the first event */
     int uniform;          /* 1 after create/reset: table uses wd=fl(1/N) (S2, reading R6) */
     int have_hist;
@@ -247,6 +248,15 @@ static int setup_integrand(oracle_ctx *c)
         c->ha = p[3];
         return ORACLE_OK;
     }
+    case ID_LO_2TO2_TAB: { /* params {sqrt_s, sqrt_shat_min, cos_cut}; the PDF comes from oracle_set_table */
+        if (c->n_params != 3 || c->dim != 3 || !is_f64(c)) return ORACLE_EINVAL;
+        double s = p[0] * p[0];
+        double smin = p[1] * p[1];
+        c->hs = s;
+        c->hL = log(smin / s);
+        c->hcut = p[2];
+        return ORACLE_OK;
+    }
     case ID_TOY_SUM:
         if (c->n_params != 0) return ORACLE_EINVAL;
         return ORACLE_OK;
@@ -295,7 +305,7 @@ void oracle_destroy(oracle_ctx *c)
 {
     if (!c) return;
     free(c->edges); free(c->hist); free(c->lo_d); free(c->wd_d); free(c->g_d);
-    free(c->lo_f); free(c->wd_f); free(c->g_f);
+    free(c->lo_f); free(c->wd_f); free(c->g_f); free(c->tab);
     free(c);
 }
 
@@ -337,6 +347,26 @@ int oracle_set_grid(oracle_ctx *c, const double *edges)
 /* ------------------------------------------------------------------------------------------------
  * S3 -- integrands, normative evaluation order.
  * ---------------------------------------------------------------------------------------------- */
+/* Tabulated PDF: M knots uniform in ln x.  x = tau^v, so ln x = v L is linear in v: knot j sits at
+ * v_j = 1 - j/(M-1), i.e. G_0 = g(tau) (v = 1) ... G_{M-1} = g(1) (v = 0).
+ * u = (1 - v)(M - 1); j = floor(u) clamped to [1, M-3]; s = u - j; four-point Lagrange (cubic) interpolation
+ *   w0 = -s(s-1)(s-2)/6, w1 = (s+1)(s-1)(s-2)/2, w2 = -(s+1)s(s-2)/2, w3 = (s+1)s(s-1)/6,
+ *   g = ((w0 G[j-1] + w1 G[j]) + w2 G[j+1]) + w3 G[j+2]          (plain products and sums, that order). */
+static double tab_interp(const double *G, int M, double v)
+{
+    double u = (1.0 - v) * (double)(M - 1);
+    int j = (int)floor(u);
+    if (j < 1) j = 1;
+    if (j > M - 3) j = M - 3;
+    double s = u - (double)j;
+    double sp = s + 1.0, sm1 = s - 1.0, sm2 = s - 2.0;
+    double w0 = -((s * sm1) * sm2) / 6.0;
+    double w1 = ((sp * sm1) * sm2) / 2.0;
+    double w2 = -((sp * s) * sm2) / 2.0;
+    double w3 = ((sp * s) * sm1) / 6.0;
+    return ((w0 * G[j - 1] + w1 * G[j]) + w2 * G[j + 1]) + w3 * G[j + 2];
+}
+
 static double eval_fp64(const oracle_ctx *c, const double *x, int *pass_out)
 {
     const int d = c->dim;
@@ -378,6 +408,28 @@ static double eval_fp64(const oracle_ctx *c, const double *x, int *pass_out)
         double Jac = (x12 * (L * L)) * 2.0;             /* |d(x1,x2,cos)/d(v1,v2,v3)| */
         return (((g1 * g2) * ME) * flux) * Jac;
     }
+    case ID_LO_2TO2_TAB: {    /* I3 with g(x) interpolated from a table (PDFFlow-style lookup,
+                               * PAPER.md:L33, L49; a synthetic table stands in for a PDF grid) */
+        const double v1 = x[0], v2 = x[1], v3 = x[2];
+        const double L = c->hL, s = c->hs;
+        double cth = fma(2.0, v3, -1.0);
+        int pass = ((v1 + v2) < 1.0) && (fabs(cth) < c->hcut);
+        *pass_out = pass;
+        if (!pass) return 0.0;
+        if (!c->tab) return NAN;
+        double x1 = exp(v1 * L);
+        double x2 = exp(v2 * L);
+        double x12 = x1 * x2;
+        double shat = x12 * s;
+        double that = (-0.5 * shat) * (1.0 - cth);
+        double uhat = (-0.5 * shat) * (1.0 + cth);
+        double ME = (shat * shat + uhat * uhat) / (that * that);
+        double g1 = tab_interp(c->tab, c->ntab, v1);
+        double g2 = tab_interp(c->tab, c->ntab, v2);
+        double flux = 1.0 / (2.0 * shat);
+        double Jac = (x12 * (L * L)) * 2.0;
+        return (((g1 * g2) * ME) * flux) * Jac;
+    }
     case ID_TOY_SUM: {        /* PAPER.md:L72-L73  tf.reduce_sum(xarr, axis=1) */
         double f = 0.0;
         for (int k = 0; k < d; ++k) f = f + x[k];
@@ -409,8 +461,6 @@ static float eval_fp32(const oracle_ctx *c, const float *x)
         for (int k = 0; k < d; ++k) f = f + x[k];
         return f;
     }
-    case ID_USER:
-        return c->user_fn ? c->user_fn(x, d, c->params) : NAN;
     default:
         return NAN;
     }
@@ -733,3 +783,19 @@ int oracle_set_user_integrand(oracle_ctx *c, oracle_user_fn fn)
     c->user_fn = fn;
     return ORACLE_OK;
 }
+
+/* ID_LO_2TO2_TAB: the tabulated PDF (M >= 4 values, copied). */
+int oracle_set_table(oracle_ctx *c, const double *values, int n)
+{
+    if (!c || !values || n < 4 || n > 4096) return ORACLE_EINVAL;
+    double *t = (double *)malloc(sizeof(double) * (size_t)n);
+    if (!t) return ORACLE_ENOMEM;
+    memcpy(t, values, sizeof(double) * (size_t)n);
+    free(c->tab);
+    c->tab = t;
+    c->ntab = n;
+    return ORACLE_OK;
+}
+
+/* the interpolation alone, for its pins */
+double oracle_tab_interp(const double *values, int n, double v) { return tab_interp(values, n, v); }

@@ -21,6 +21,7 @@ namespace {
 
 using namespace vegas;
 
+constexpr int kMaxTable = 4096;         // doubles of integrand data (tabulated PDF)
 constexpr int kRing = 64;               // (I, sigma) entries logged on the device between two reads of a graph run
 constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
 constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
@@ -50,7 +51,7 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ---- device workspace layout (all offsets 256-byte aligned) -------------------------------------
 struct Layout {
-    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, dev_iter, ring, total;
+    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, dev_iter, ring, idata, total;
 };
 
 Layout make_layout(int dim, int nbins)
@@ -71,6 +72,7 @@ Layout make_layout(int dim, int nbins)
     L.status = o;     o = align_up(o + 4, 256);
     L.dev_iter = o;   o = align_up(o + 4, 256);                    // iteration counter of CUDA-graph replays
     L.ring = o;       o = align_up(o + static_cast<size_t>(kRing) * 16, 256);   // their (I, sigma) log
+    L.idata = o;      o = align_up(o + static_cast<size_t>(kMaxTable) * 8, 256);     // integrand data (vegas_set_table)
     L.total = o;
     return L;
 }
@@ -169,6 +171,8 @@ const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, 100, 3, 4, 0, VEGAS_FP32_EVAL, 1024, 1, 1024),  // configs[3]
     VEGAS_TUNED(VEGAS_LO_2TO2, Lo2to2, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),                // configs[4]
     VEGAS_TUNED(VEGAS_GAUSS_DOUBLE, U32<GaussDouble>, 8, 50, 5, 8, 4, VEGAS_FP64_U32, 768, 1, 768),   // configs[1] with 32-bit uniforms
+    VEGAS_TUNED(VEGAS_LO_2TO2_TAB, Lo2to2Tab, 3, 50, 5, 8, 3, VEGAS_FP64, 1024, 2, 1024),         // NEXT-4
+    VEGAS_GENERIC(VEGAS_LO_2TO2_TAB, Lo2to2Tab, 3, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GAUSS_SYM, GaussSym, 4, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GAUSS_DOUBLE, GaussDouble, 8, VEGAS_FP64),
     VEGAS_GENERIC(VEGAS_GENZ_OSC_PEAK, GenzOscPeak, 20, VEGAS_FP32_EVAL),
@@ -211,6 +215,7 @@ int expected_params(int id, int dim)
         case VEGAS_GENZ_OSC_PEAK: return 1 + dim;
         case VEGAS_LO_2TO2: return 5;
         case VEGAS_TOY_SUM: return 0;
+        case VEGAS_LO_2TO2_TAB: return 3;
         case VEGAS_USER: return -2;          // any count up to kMaxUserParams (checked by vegas_create_custom)
         default: return -1;
     }
@@ -293,6 +298,17 @@ int setup_integrand(vegas_ctx* c, const double* p)
             c->ic.hcut = p[2];
             c->ic.ha = p[3];
             c->ic.hLLs = (c->ic.hL * c->ic.hL) / s;
+            return VEGAS_OK;
+        }
+        case VEGAS_LO_2TO2_TAB: {
+            if (c->dim != 3) return fail(VEGAS_EINVAL, "lo_2to2_tab needs dim = 3");
+            const double s = p[0] * p[0];
+            c->ic.hs = s;
+            c->ic.hL = std::log((p[1] * p[1]) / s);
+            c->ic.hcut = p[2];
+            c->ic.hLLs = (c->ic.hL * c->ic.hL) / s;
+            c->ic.tab = nullptr;                          // vegas_set_table
+            c->ic.ntab = 0;
             return VEGAS_OK;
         }
         case VEGAS_USER:
@@ -603,6 +619,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (n_events < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
+    if (c->integrand_id == VEGAS_LO_2TO2_TAB && !c->ic.tab) return fail(VEGAS_ESTATE, "lo_2to2_tab needs vegas_set_table first");
     if (events_per_launch == 0) return fail(VEGAS_EINVAL, "events_per_launch must be > 0");
     if (n_events > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
     const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
@@ -916,6 +933,19 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     c->refine_pending = total;
     rc = vegas_refine_collect(c);
     return rc == VEGAS_EGRID ? VEGAS_OK : rc;            // a rejected refinement left its grid unchanged; the run went on
+}
+
+int vegas_set_table(vegas_ctx* c, const double* values, int n)
+{
+    if (!c || !values) return fail(VEGAS_EINVAL, "NULL argument");
+    if (c->integrand_id != VEGAS_LO_2TO2_TAB) return fail(VEGAS_EINVAL, "this integrand takes no table");
+    if (n < 4 || n > kMaxTable) return fail(VEGAS_EINVAL, "table length %d not in 4..%d", n, kMaxTable);
+    CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.idata, values, sizeof(double) * static_cast<size_t>(n), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));          // `values` is pageable host memory owned by the caller
+    c->ic.tab = reinterpret_cast<const double*>(c->ws + c->L.idata);
+    c->ic.ntab = n;
+    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }   // captured kernel arguments are stale
+    return VEGAS_OK;
 }
 
 int vegas_use_cuda_graph(vegas_ctx* c, int enable)

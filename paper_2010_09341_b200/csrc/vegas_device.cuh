@@ -39,6 +39,9 @@ struct IntegrandConsts {
     float zw[kMaxDim];
     // user integrand compiled at run time (vegas_create_custom): its parameters
     double user_params[16];
+    // lo_2to2_tab: the tabulated PDF (device pointer into the workspace, vegas_set_table) and its length
+    const double* tab;
+    int ntab;
 };
 
 constexpr int kMaxUserParams = 16;
@@ -253,6 +256,41 @@ struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, 
         const double opc = __dadd_rn(1.0, cth), omc = __dsub_rn(1.0, cth);
         const double ME = __ddiv_rn(__fma_rn(opc, opc, 4.0), __dmul_rn(omc, omc));
         return __dmul_rn(__dmul_rn(__dmul_rn(e12, y5), ME), c.hLLs);
+    }
+};
+
+// Four-point Lagrange (cubic) interpolation of a table with knots uniform in ln x: x = tau^v, knot j at
+// v_j = 1 - j/(M-1).  u = (1-v)(M-1), j = floor(u) clamped to [1, M-3], s = u - j,
+//   g = ((w0 G[j-1] + w1 G[j]) + w2 G[j+1]) + w3 G[j+2],  w0 = -s(s-1)(s-2)/6, w1 = (s+1)(s-1)(s-2)/2,
+//   w2 = -(s+1)s(s-2)/2, w3 = (s+1)s(s-1)/6 -- plain products and sums in this order (no contraction), so
+// the value is bit-identical to the CPU statement of the same recipe.  The four loads are L1/L2-resident global
+// reads (the table is a few KB): this is the PDFFlow-style gather of PAPER.md:L33, L49.
+__device__ __forceinline__ double tab_interp(const double* __restrict__ G, int M, double v)
+{
+    const double u = __dmul_rn(__dsub_rn(1.0, v), static_cast<double>(M - 1));
+    int j = static_cast<int>(floor(u));
+    j = j < 1 ? 1 : (j > M - 3 ? M - 3 : j);
+    const double s = __dsub_rn(u, static_cast<double>(j));
+    const double sp = __dadd_rn(s, 1.0), sm1 = __dsub_rn(s, 1.0), sm2 = __dsub_rn(s, 2.0);
+    const double w0 = __ddiv_rn(-__dmul_rn(__dmul_rn(s, sm1), sm2), 6.0);
+    const double w1 = __ddiv_rn(__dmul_rn(__dmul_rn(sp, sm1), sm2), 2.0);
+    const double w2 = __ddiv_rn(-__dmul_rn(__dmul_rn(sp, s), sm2), 2.0);
+    const double w3 = __ddiv_rn(__dmul_rn(__dmul_rn(sp, s), sm1), 6.0);
+    const double g0 = __ldg(G + j - 1), g1 = __ldg(G + j), g2 = __ldg(G + j + 1), g3 = __ldg(G + j + 2);
+    return __dadd_rn(__dadd_rn(__dadd_rn(__dmul_rn(w0, g0), __dmul_rn(w1, g1)), __dmul_rn(w2, g2)), __dmul_rn(w3, g3));
+}
+
+struct Lo2to2Tab : Lo2to2 {  // NEXT-4: lo_2to2 with the PDF g(x) interpolated from a table (id 6)
+    static constexpr int kId = 6;
+    // f = g(x1) g(x2) ME flux Jac in the reduced form of Lo2to2::end (shat cancels): g1 g2 (4+(1+c)^2)/(1-c)^2 L^2/s
+    __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
+    {
+        const double cth = __fma_rn(2.0, v[2], -1.0);
+        const double g1 = tab_interp(c.tab, c.ntab, v[0]);
+        const double g2 = tab_interp(c.tab, c.ntab, v[1]);
+        const double opc = __dadd_rn(1.0, cth), omc = __dsub_rn(1.0, cth);
+        const double ME = __ddiv_rn(__fma_rn(opc, opc, 4.0), __dmul_rn(omc, omc));
+        return __dmul_rn(__dmul_rn(__dmul_rn(g1, g2), ME), c.hLLs);
     }
 };
 

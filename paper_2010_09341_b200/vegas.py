@@ -15,7 +15,7 @@ from . import build as _build
 
 OK, EINVAL, ECUDA, ENOMEM, ESTATE, EUNSUPPORTED, EGRID = 0, -1, -2, -3, -4, -5, -6
 FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
-GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM, USER = 0, 1, 2, 3, 4, 5
+GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM, USER, LO_2TO2_TAB = 0, 1, 2, 3, 4, 5, 6
 
 _vp, _dp, _ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
 _i32p, _u32p, _u64p, _szp = C.POINTER(C.c_int32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint64), C.POINTER(C.c_size_t)
@@ -30,6 +30,7 @@ SIGNATURES = {
     "vegas_refine_enqueue": (C.c_int, [_vp, C.c_double]),
     "vegas_refine_collect": (C.c_int, [_vp]),
     "vegas_iteration_kernel_ms": (C.c_int, [_vp, C.c_int, _dp]),
+    "vegas_set_table": (C.c_int, [_vp, _dp, C.c_int]),
     "vegas_get_grid": (C.c_int, [_vp, _dp]),
     "vegas_set_grid": (C.c_int, [_vp, _dp]),
     "vegas_reset": (C.c_int, [_vp]),
@@ -203,6 +204,10 @@ class Vegas:
         e = np.ascontiguousarray(edges, dtype=np.float64)
         assert e.shape == (self.dim, self.nbins + 1)
         _chk(lib().vegas_set_grid(self._h, _d(e)), "vegas_set_grid")
+
+    def set_table(self, values):
+        v = np.ascontiguousarray(values, dtype=np.float64)
+        _chk(lib().vegas_set_table(self._h, _d(v), int(v.size)), "vegas_set_table")
 
     def reset(self):
         _chk(lib().vegas_reset(self._h), "vegas_reset")

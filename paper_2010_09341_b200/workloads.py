@@ -17,7 +17,7 @@ from dataclasses import dataclass, field
 from typing import Tuple
 
 # integrand ids and precisions of the C ABI (include/vegas_b200.h)
-GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM = 0, 1, 2, 3, 4
+GAUSS_SYM, GAUSS_DOUBLE, GENZ_OSC_PEAK, LO_2TO2, TOY_SUM, USER, LO_2TO2_TAB = 0, 1, 2, 3, 4, 5, 6
 FP64, FP32_EVAL, FP64_U32 = 0, 1, 2
 
 _M32 = 0xFFFFFFFF
@@ -94,10 +94,29 @@ def cfg5(n_events=10**8, n_iter=10):
                     n_events, n_iter, note="BASELINE.json configs[4]")
 
 
+def pdf_table(n_knots=1024, sqrt_s=13000.0, sqrt_shat_min=50.0, a=1.1, b=5):
+    """Synthetic PDF grid for lo_2to2_tab: values[j] = g(x_j) = x_j^-a (1-x_j)^b at x_j = tau^(1 - j/(n-1)) -- the toy PDF
+    of BASELINE.json configs[4] tabulated on knots uniform in ln x (a stand-in for a PDFFlow/LHAPDF grid, which is not
+    available).  Input data only: the interpolation is done by the CUDA path and by the oracle, each on its own."""
+    import math
+    tau = (sqrt_shat_min / sqrt_s) ** 2
+    out = []
+    for j in range(n_knots):
+        x = 1.0 if j == n_knots - 1 else math.exp((1.0 - j / (n_knots - 1.0)) * math.log(tau))
+        out.append(x ** (-a) * (1.0 - x) ** b)
+    return out
+
+
+def cfg5_tab(n_events=10**8, n_iter=10):
+    """NEXT-4: configs[4] with the PDF looked up in a 1024-knot table instead of evaluated analytically."""
+    return Workload("cfg5_lo_2to2_tab_d3", 3, 50, LO_2TO2_TAB, (13000.0, 50.0, 0.9), FP64, n_events, n_iter,
+                    note="BASELINE.json configs[4] with a tabulated PDF (SURVEY 8.f NEXT-4)")
+
+
 def toy(dim=10):
     """f = sum_i x_i, n_dim=10, n_events=1e6, events_limit=1e5, n_iter=5."""
     return Workload("toy_sum_d%d" % dim, dim, 50, TOY_SUM, (), FP64, 10**6, 5, events_per_launch=10**5,
                     note="PAPER.md:L72-L79 usage example")
 
 
-ALL = {"cfg1": cfg1, "cfg2": cfg2, "cfg2_u32": cfg2_u32, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5, "toy": toy}
+ALL = {"cfg1": cfg1, "cfg2": cfg2, "cfg2_u32": cfg2_u32, "cfg5_tab": cfg5_tab, "cfg3": cfg3, "cfg4": cfg4, "cfg5": cfg5, "toy": toy}

@@ -40,6 +40,7 @@ def small_workloads():
         "toy_d32": W.Workload("toy32", 32, 50, W.TOY_SUM, (), W.FP64, 10**5, 3),
         "toy_f32_d9": W.Workload("toyf9", 9, 100, W.TOY_SUM, (), W.FP32_EVAL, 10**5, 3),
         # 32-bit-uniform stream mode (extra; reading R3): tuned and generic instances
+        "cfg5_tab": W.cfg5_tab(),                        # NEXT-4: tabulated PDF
         "cfg2_u32": W.cfg2_u32(),
         "lo_u32": W.Workload("lo_u32", 3, 50, W.LO_2TO2, (13000.0, 50.0, 0.9, 1.1, 5.0), W.FP64_U32, 10**5, 3),
         "gauss_sym_d5_u32": W.Workload("gs5u", 5, 33, W.GAUSS_SYM, (0.1, 0.5), W.FP64_U32, 10**5, 3),
@@ -47,11 +48,15 @@ def small_workloads():
     }
 
 
-F_RTOL = {W.GAUSS_SYM: 2e-15, W.GAUSS_DOUBLE: 2e-15, W.GENZ_OSC_PEAK: 0.0, W.LO_2TO2: 2e-14, W.TOY_SUM: 0.0}
+F_RTOL = {W.GAUSS_SYM: 2e-15, W.GAUSS_DOUBLE: 2e-15, W.GENZ_OSC_PEAK: 0.0, W.LO_2TO2: 2e-14, W.TOY_SUM: 0.0,
+          W.LO_2TO2_TAB: 2e-14}
 
 
 def make_pair(V, O, w):
-    return V.from_workload(w), O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    g, o = V.from_workload(w), O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    if w.integrand_id == W.LO_2TO2_TAB:                 # the tabulated PDF is input data for both sides
+        g.set_table(W.pdf_table()); o.set_table(W.pdf_table())
+    return g, o
 
 
 def assert_events_equal(g, o, w):
@@ -180,7 +185,7 @@ def test_cfg1_full_five_iterations(V, O):
     run_cascade(g, o, w, w.n_events, w.n_iter)
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "toy", "gauss_sym_d2", "toy_f32_d9", "cfg2_u32", "lo_u32"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "toy", "gauss_sym_d2", "toy_f32_d9", "cfg2_u32", "lo_u32", "cfg5_tab"])
 def test_cascade_reduced(V, O, name):
     w = small_workloads()[name]
     g, o = make_pair(V, O, w)
@@ -314,7 +319,7 @@ def test_estimates_within_4_sigma_of_closed_form(V, golden_dir):
 # BASELINE.json full sizes, in the launch configuration bench.py times (one launch per iteration, the
 # instance's default shape)
 # ---------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "cfg2_u32"])
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5", "cfg2_u32", "cfg5_tab"])
 def test_full_size_iteration_parity(V, O, name):
     """1e8 events: iteration 0 on the uniform grid and iteration 1 on the oracle's refined grid
     (cascade-free), I / sigma rel 1e-12, every histogram cell rel 1e-10, pass count exact, plus sampled events
