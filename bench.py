@@ -40,9 +40,9 @@ ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg2_u32": 154.0, "cfg4": 232.0, "cf
 # FP pipe lanes per SM (B200): 64 fp64, 128 fp32.  Peak = SMs * lanes * 2 FLOP * max SM clock.
 FP_LANES = {"f64": 64, "f32": 128}
 # dram__bytes_read.sum + dram__bytes_write.sum of one 1e8-event iterate_kernel launch, from the ncu --set full
-# captures summarised in profiles/r01c_ncu_full_<cfg>_iterate.md (the algorithmic HBM traffic is ~0: one table
+# captures summarised in profiles/r01[c-e]_ncu_full_<cfg>_iterate.md (the algorithmic HBM traffic is ~0: one table
 # read and one d*N flush per CTA)
-NCU_TRAFFIC_BYTES = {"cfg2": 36352, "cfg4": 73216, "cfg5": 44032}
+NCU_TRAFFIC_BYTES = {"cfg2": 36352, "cfg4": 73216, "cfg5": 44032}   # r01c-r01e captures: 35-44 KB (cfg2, cfg5), 70-73 KB (cfg4)
 
 
 def parse_args():
