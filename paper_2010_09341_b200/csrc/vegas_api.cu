@@ -636,6 +636,12 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
     // launches that do not fill the GPU overlap, and every launch's prologue/flush overlaps its neighbours'.
     const uint64_t n_launches = (n_events + epl - 1) / epl;
     const int lanes = n_launches > 1 ? kLanes : 1;
+    // several launches in flight: each takes a fraction of the SMs, so that one launch's prologue / flush overlaps
+    // its neighbours' event loops (a CTA of a tuned instance fills an SM's shared memory: full-size grids cannot
+    // share an SM).  The fraction grows with the number of launches (measured on cfg3: 2.03 / 2.16 / 3.11 ms per
+    // 1e8 events at 1e7 / 1e6 / 1e5 events per launch with 1/2, 1/4, 1/8 of the SMs, against 2.06 / 2.52 / 5.83).
+    const int split = n_launches >= 512 ? 8 : n_launches >= 32 ? 4 : n_launches >= 8 ? 2 : 1;
+    const int cap_grid = (max_grid + split - 1) / split;
     if (lanes > 1) {
         CUDA_TRY(cudaEventRecord(c->fork, c->stream));
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
@@ -651,7 +657,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
         a.e_hi = static_cast<uint32_t>(done >> 32);
         a.count = static_cast<uint32_t>(cnt);
         const uint64_t want = (cnt + c->threads - 1) / c->threads;
-        const int grid = want < static_cast<uint64_t>(max_grid) ? static_cast<int>(want) : max_grid;
+        const int grid = want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
         const int ln = launches % lanes;
         a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
         CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
