@@ -230,7 +230,7 @@ def run_b200(args):
     def step_async():
         nl = g.iterate_enqueue(n, epl, w.seed)
         g.refine_enqueue(w.alpha)           # S7, no host round trip; outcome collected after the timed region
-        return nl + 2
+        return nl + 1                       # iterate launches (S6 runs in their last CTA) + the refine kernel
 
     # ---- device-timed region ----
     g.reset()

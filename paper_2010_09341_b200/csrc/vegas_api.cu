@@ -69,7 +69,7 @@ Layout make_layout(int dim, int nbins)
     L.zero_end = o;
     L.result = o;     o = align_up(o + 64, 256);
     L.flags = o;      o = align_up(o + kMaxDim * 4, 256);
-    L.status = o;     o = align_up(o + 4, 256);
+    L.status = o;     o = align_up(o + 8, 256);                    // refine status word + ticket counter
     L.dev_iter = o;   o = align_up(o + 4, 256);                    // iteration counter of CUDA-graph replays
     L.ring = o;       o = align_up(o + static_cast<size_t>(kRing) * 16, 256);   // their (I, sigma) log
     L.idata = o;      o = align_up(o + static_cast<size_t>(kMaxTable) * 8, 256);     // integrand data (vegas_set_table)
@@ -375,6 +375,8 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
     a.count = count;
     a.iteration = c->iteration;
     a.iter_ptr = nullptr;
+    a.ticket = nullptr; a.total_ctas = 0; a.slots0 = nullptr; a.fin_lanes = 0; a.fin_stride = 0; a.fin_used = 0;
+    a.n_events = 0; a.result = nullptr; a.dev_iter = nullptr; a.ring = nullptr; a.ring_len = 0;
     const uint32_t k0 = static_cast<uint32_t>(seed), k1 = static_cast<uint32_t>(seed >> 32);
     for (int r = 0; r < 10; ++r) {
         a.rk0[r] = k0 + static_cast<uint32_t>(r) * 0x9E3779B9u;
@@ -647,21 +649,47 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
     }
     double* slots0 = reinterpret_cast<double*>(c->ws + c->L.slots);
-    int launches = 0, used_grid = 0;
-    for (uint64_t done = 0; done < n_events;) {
+    // launch geometry of the whole iteration first: S6 runs in the CTA that finishes last, so every launch must
+    // know how many CTAs there are in total and how many slots each stream-lane region uses
+    auto launch_count = [&](uint64_t done) {
         uint64_t cnt = n_events - done;
         if (cnt > epl) cnt = epl;
         const uint64_t to_wrap = (uint64_t(1) << 32) - (done & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
-        if (cnt > to_wrap) cnt = to_wrap;
+        return cnt > to_wrap ? to_wrap : cnt;
+    };
+    auto launch_grid = [&](uint64_t cnt) {
+        const uint64_t want = (cnt + c->threads - 1) / c->threads;
+        return want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
+    };
+    uint64_t total_ctas = 0;
+    int used_grid = 0;
+    for (uint64_t done = 0; done < n_events;) {
+        const uint64_t cnt = launch_count(done);
+        const int grid = launch_grid(cnt);
+        total_ctas += static_cast<uint64_t>(grid);
+        if (grid > used_grid) used_grid = grid;
+        done += cnt;
+    }
+    if (total_ctas > 0xFFFFFFFFull) return fail(VEGAS_EINVAL, "too many launches for one iteration (raise events_per_launch)");
+    a.ticket = reinterpret_cast<unsigned int*>(c->ws + c->L.npass) + 4;   // inside the region cleared by the memset
+    a.total_ctas = static_cast<unsigned int>(total_ctas);
+    a.slots0 = slots0;
+    a.fin_lanes = lanes; a.fin_stride = kLaneSlots; a.fin_used = used_grid;
+    a.n_events = n_events;
+    a.result = reinterpret_cast<double*>(c->ws + c->L.result);
+    a.dev_iter = graph_mode ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr;
+    a.ring = graph_mode ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr;
+    a.ring_len = kRing;
+    int launches = 0;
+    for (uint64_t done = 0; done < n_events;) {
+        const uint64_t cnt = launch_count(done);
         a.e_lo_first = static_cast<uint32_t>(done);
         a.e_hi = static_cast<uint32_t>(done >> 32);
         a.count = static_cast<uint32_t>(cnt);
-        const uint64_t want = (cnt + c->threads - 1) / c->threads;
-        const int grid = want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
+        const int grid = launch_grid(cnt);
         const int ln = launches % lanes;
         a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
         CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
-        if (grid > used_grid) used_grid = grid;
         done += cnt;
         ++launches;
     }
@@ -671,15 +699,10 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
             CUDA_TRY(cudaStreamWaitEvent(c->stream, c->lane_done[i], 0));
         }
     }
-    finalize_kernel<<<1, 32, 0, c->stream>>>(slots0, lanes, kLaneSlots, used_grid,
-                                             reinterpret_cast<const unsigned long long*>(c->ws + c->L.npass),
-                                             n_events, reinterpret_cast<double*>(c->ws + c->L.result),
-                                             graph_mode ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr,
-                                             graph_mode ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr, kRing);
     CUDA_TRY(cudaGetLastError());
-    if (n_kernel_launches) *n_kernel_launches = launches + 1;
+    if (n_kernel_launches) *n_kernel_launches = launches;
     c->have_hist = true;
-    c->last_launches = launches + 1;
+    c->last_launches = launches;
     if (graph_mode) return VEGAS_OK;
     CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
     c->n_enqueued += 1;
@@ -687,8 +710,8 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
     c->have_hist = true;
     c->have_sums = true;
     c->last_n = n_events;
-    c->last_launches = launches + 1;
-    if (n_kernel_launches) *n_kernel_launches = launches + 1;
+    c->last_launches = launches;
+    if (n_kernel_launches) *n_kernel_launches = launches;
     return VEGAS_OK;
 }
 
@@ -757,10 +780,9 @@ int vegas_refine_enqueue(vegas_ctx* c, double alpha)
     double* hist = reinterpret_cast<double*>(c->ws + c->L.hist);
     int* flags = reinterpret_cast<int*>(c->ws + c->L.flags);
     int* status = reinterpret_cast<int*>(c->ws + c->L.status);
-    refine_kernel<<<c->dim, 128, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags);
-    CUDA_TRY(cudaGetLastError());
-    refine_commit_kernel<<<c->dim, 128, 0, c->stream>>>(edges, new_edges, flags, c->dim, N, c->ws + c->L.table,
-                                                        c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status);
+    refine_kernel<<<c->dim, 128, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags, c->dim, c->ws + c->L.table,
+                                                    c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status,
+                                                    reinterpret_cast<unsigned int*>(c->ws + c->L.status) + 1);
     CUDA_TRY(cudaGetLastError());
     c->have_hist = false;
     c->refine_pending += 1;

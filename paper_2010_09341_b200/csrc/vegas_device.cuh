@@ -56,6 +56,16 @@ struct IterArgs {
     uint32_t count;        // events in this launch (<= 2^31)
     uint32_t iteration;    // Philox counter word 2 (used when iter_ptr is NULL)
     const uint32_t* iter_ptr;  // device: the counter lives in memory (CUDA-graph replays of run_integration)
+    // S6 runs in the CTA that finishes last over all launches of the iteration (ticket counter):
+    unsigned int* ticket;      // device: CTAs finished so far (zeroed with the accumulators)
+    unsigned int total_ctas;   // CTAs of all launches of this iteration
+    double* slots0;            // base of the slot regions; fin_lanes regions of stride fin_stride, fin_used slots each
+    int fin_lanes, fin_stride, fin_used;
+    unsigned long long n_events;
+    double* result;            // device: I, sigma, S1, S2, npass, n
+    uint32_t* dev_iter;        // graph replays: advanced by S6 (NULL otherwise)
+    double* ring;              // graph replays: (I, sigma) log (NULL otherwise)
+    int ring_len;
     uint32_t rk0[10], rk1[10];  // Philox round keys: k + r * Weyl
     int dim, nbins;
     int rshift;            // log2 of the number R of lane-indexed histogram replicas in shared memory

@@ -132,6 +132,10 @@ __device__ __forceinline__ void hist_update_batch(double* hlane, int k0, int d, 
     }
 }
 
+__device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, int lane_stride, int per_lane,
+                                              const unsigned long long* npass, unsigned long long n_events,
+                                              double* result, uint32_t* dev_iter, double* ring, int ring_len);
+
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
 {
@@ -294,27 +298,40 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
         for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[(r + c) & (R - 1)]);
         if (v != 0.0) atomicAdd(a.hist + c, v);
     }
+
+    // ---- S6 in the CTA that finishes last over all launches of this iteration ----
+    __shared__ int sh_last;
+    __syncthreads();                                     // this CTA's slot is written
+    if (tid == 0) {
+        __threadfence();
+        sh_last = (atomicAdd(a.ticket, 1u) == a.total_ctas - 1u);
+    }
+    __syncthreads();
+    if (sh_last && tid < 32) {
+        __threadfence();                                 // see the other CTAs' slots
+        finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.result, a.dev_iter, a.ring,
+                      a.ring_len);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
-// finalize_kernel (S6): fixed-order compensated sum of the per-CTA slots, then
+// finalize_warp (S6), run by the first warp of the CTA that finishes last: fixed-order compensated sum of the
+// per-CTA slots, then
 //   I = S1/n ; V = (S2/n - I*I)/(n-1) ; sigma = sqrt(max(V, 0)).
 // One warp; lane l folds slots l, l+32, ... (over the per-stream-lane regions) then a shuffle tree: the order
 // depends only on the launch geometry.
 // result[0..5] = I, sigma, S1, S2, npass, n
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__ slots, int nlanes, int lane_stride,
-                                                      int per_lane,
-                                                      const unsigned long long* __restrict__ npass,
-                                                      unsigned long long n_events, double* __restrict__ result,
-                                                      uint32_t* dev_iter, double* __restrict__ ring, int ring_len)
+__device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, int lane_stride, int per_lane,
+                                              const unsigned long long* npass, unsigned long long n_events,
+                                              double* result, uint32_t* dev_iter, double* ring, int ring_len)
 {
-    const int lane = threadIdx.x;
+    const int lane = threadIdx.x & 31;
     Comp t1{0.0, 0.0}, t2{0.0, 0.0};
     for (int e = lane; e < nlanes * per_lane; e += 32) {         // slot region of stream-lane e / per_lane
         const size_t s = static_cast<size_t>(e / per_lane) * lane_stride + (e % per_lane);
-        comp_add(t1, slots[s * 4 + 0], slots[s * 4 + 1]);
-        comp_add(t2, slots[s * 4 + 2], slots[s * 4 + 3]);
+        comp_add(t1, __ldcg(slots + s * 4 + 0), __ldcg(slots + s * 4 + 1));   // written by other CTAs: L2 reads
+        comp_add(t2, __ldcg(slots + s * 4 + 2), __ldcg(slots + s * 4 + 3));
     }
     comp_warp_reduce(t1);
     comp_warp_reduce(t2);
@@ -327,7 +344,7 @@ __global__ void __launch_bounds__(32) finalize_kernel(const double* __restrict__
         result[1] = sqrt(V > 0.0 ? V : 0.0);
         result[2] = S1;
         result[3] = S2;
-        result[4] = static_cast<double>(*npass);
+        result[4] = static_cast<double>(__ldcg(npass));
         result[5] = n;
         if (ring) {                                      // graph replays: log (I, sigma) and advance the counter
             const uint32_t it = *dev_iter;
@@ -373,8 +390,8 @@ __global__ void build_table_kernel(double* __restrict__ edges, void* __restrict_
 // prefix sums are sequential in ascending i (one thread), exactly the order the definition states; the
 // per-bin work (smoothing, damping, edge interpolation) is spread over the threads.
 //   new_edges[k][*] receives the candidate edges; flags[k] = 0 ok / 1 not strictly increasing.
-__global__ void refine_kernel(const double* __restrict__ edges, const double* __restrict__ hist, int N,
-                              double alpha, double* __restrict__ new_edges, int* __restrict__ flags)
+__device__ __forceinline__ void refine_dimension(const double* edges, const double* hist, int N, double alpha,
+                                                 double* new_edges, int* flags)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double* s = reinterpret_cast<double*>(smem_raw);   // [N]   smoothed
@@ -452,27 +469,40 @@ __global__ void refine_kernel(const double* __restrict__ edges, const double* __
     if (tid == 0) flags[k] = sh_bad;
 }
 
-// commit (S7 step 7): if every dimension passed, the candidate edges become the master edges, the table
-// is rebuilt and H is cleared; otherwise nothing changes.  status[0] is set to 1 on a rejection (sticky: the
-// host clears it when it collects the outcome of the refinements enqueued since).
-__global__ void refine_commit_kernel(double* __restrict__ edges, const double* __restrict__ new_edges,
-                                     const int* __restrict__ flags, int d, int N, void* __restrict__ table,
-                                     int precision, double* __restrict__ hist, int* __restrict__ status)
+// refine_kernel (S7): one CTA per dimension computes that dimension's candidate edges (refine_dimension); the
+// CTA that finishes last (ticket counter, __threadfence) does step 7 for all dimensions: if every dimension passed,
+// the candidate edges become the master edges, the table is rebuilt and H is cleared; otherwise nothing changes and
+// status[0] is set to 1 (sticky: the host clears it when it collects the outcome of the refinements enqueued since).
+// One launch instead of two: the all-or-nothing commit needs every dimension's flag, i.e. a grid-wide dependency.
+__global__ void refine_kernel(double* edges, const double* hist_in, int N, double alpha, double* new_edges, int* flags,
+                              int d, void* table, int precision, double* hist, int* status, unsigned int* ticket)
 {
-    const int k = blockIdx.x;
-    int bad = 0;
-    for (int j = 0; j < d; ++j) bad |= flags[j];
-    if (threadIdx.x == 0 && k == 0 && bad) status[0] = 1;   // sticky until the host collects and clears it
-    if (bad) return;
-    double* E = edges + static_cast<size_t>(k) * (N + 1);
-    const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
-    for (int i = threadIdx.x; i < N; i += blockDim.x) {
-        const double lo = En[i], hi = En[i + 1];
-        write_table_cell(table, precision, static_cast<size_t>(k) * N + i, lo, __dsub_rn(hi, lo));
-        hist[static_cast<size_t>(k) * N + i] = 0.0;
+    __shared__ int sh_last;
+    refine_dimension(edges, hist_in, N, alpha, new_edges, flags);
+    __syncthreads();                                     // this CTA's candidate edges and flag are written
+    if (threadIdx.x == 0) {
+        __threadfence();
+        sh_last = (atomicAdd(ticket, 1u) == static_cast<unsigned int>(d - 1));
     }
     __syncthreads();
-    for (int i = threadIdx.x; i <= N; i += blockDim.x) E[i] = En[i];
+    if (!sh_last) return;
+    __threadfence();                                     // see the other CTAs' edges and flags
+    int bad = 0;
+    for (int j = 0; j < d; ++j) bad |= __ldcg(flags + j);
+    if (threadIdx.x == 0) {
+        *ticket = 0u;                                    // ready for the next refinement
+        if (bad) status[0] = 1;
+    }
+    if (bad) return;
+    const int cells = d * N;
+    for (int c = threadIdx.x; c < cells; c += blockDim.x) {
+        const int k = c / N, i = c - k * N;
+        const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
+        const double lo = __ldcg(En + i), hi = __ldcg(En + i + 1);
+        write_table_cell(table, precision, static_cast<size_t>(c), lo, __dsub_rn(hi, lo));
+        hist[c] = 0.0;
+    }
+    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = __ldcg(new_edges + e);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -41,7 +41,7 @@ def run_config(name, w, n_iter=None, epl=0, tune=False):
         g.refine_enqueue(w.alpha)
         e1.record()
         g.refine_collect()
-        rms.append(e0.elapsed_time(e1))     # refine_kernel + refine_commit_kernel on the current stream
+        rms.append(e0.elapsed_time(e1))     # refine_kernel on the current stream
     out = {"config": name, "workload": w.name, "n_events": w.n_events, "events_per_launch": epl or w.n_events,
            "iterations": n_iter, "kernel_ms_median": statistics.median(ms), "kernel_ms_best": min(ms),
            "events_per_s_median": w.n_events / (statistics.median(ms) * 1e-3),
