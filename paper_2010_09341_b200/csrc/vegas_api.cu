@@ -547,6 +547,11 @@ int vegas_create_custom(vegas_ctx** out, int dim, int nbins, const char* source,
 void vegas_destroy(vegas_ctx* c)
 {
     if (!c) return;
+    // asynchronous work (enqueued iterations / refinements, graph replays) may still use the pinned buffers
+    if (c->gstream) cudaStreamSynchronize(c->gstream);
+    for (int i = 0; i < kLanes; ++i) if (c->lane[i]) cudaStreamSynchronize(c->lane[i]);
+    if (c->h_result) cudaStreamSynchronize(c->stream);
+    (void)cudaGetLastError();
     if (c->h_result) cudaFreeHost(c->h_result);
     if (c->h_status) cudaFreeHost(c->h_status);
     if (c->h_ring) cudaFreeHost(c->h_ring);
