@@ -15,7 +15,8 @@
  *   - The caller owns every buffer it passes.  `params` is copied at create.  `dev_workspace` (device
  *     memory, >= vegas_workspace_bytes(), 256-byte aligned) and `cuda_stream` (a cudaStream_t cast to
  *     void*, NULL = the legacy default stream) are borrowed and must outlive the context; the library
- *     allocates no device memory itself except a few bytes of pinned host memory for results.
+ *     allocates no device memory itself (every device buffer, the scratch of vegas_debug_events included, is a
+ *     region of dev_workspace); it allocates a few hundred bytes of pinned host memory for results.
  *   - A context is not thread-safe.  Calls that return results to host pointers are synchronous at
  *     return (they synchronise the stream); they enqueue asynchronously inside (no host sync between
  *     the launches of one iteration).
@@ -39,8 +40,8 @@ enum {
     VEGAS_EINVAL = -1,       /* bad argument (range, NULL, wrong n_params) */
     VEGAS_ECUDA = -2,        /* a CUDA runtime call failed / no device */
     VEGAS_ENOMEM = -3,       /* workspace too small or host allocation failed */
-    VEGAS_ESTATE = -4,       /* call order: vegas_refine before any vegas_iterate */
-    VEGAS_EUNSUPPORTED = -5, /* no compiled kernel instance for (integrand_id, dim, nbins, precision) */
+    VEGAS_ESTATE = -4,       /* call order: e.g. vegas_refine before any vegas_iterate */
+    VEGAS_EUNSUPPORTED = -5, /* no compiled kernel instance for (integrand_id, dim, precision); device is not sm_100 */
     VEGAS_EGRID = -6         /* grid not strictly increasing from 0 to 1; grid left unchanged */
 };
 
@@ -75,7 +76,8 @@ size_t vegas_workspace_bytes(int dim, int nbins);
  * among the compiled instances instead of being traced.
  *   dim 1..32; nbins 2..4095 (fp64) / 2..511 (fp32) so that m*nbins is exact (S2).
  * Errors: VEGAS_EINVAL (ranges, NULL out, n_params mismatch, misaligned workspace), VEGAS_ENOMEM
- * (workspace_bytes too small), VEGAS_EUNSUPPORTED (no instance), VEGAS_ECUDA. */
+ * (workspace_bytes too small), VEGAS_EUNSUPPORTED (no instance; a device other than sm_100: the library carries
+ * sm_100a code only), VEGAS_ECUDA. */
 int vegas_create(vegas_ctx** out, int dim, int nbins, int integrand_id, const double* params, int n_params,
                  int precision, void* dev_workspace, size_t workspace_bytes, void* cuda_stream);
 
@@ -113,14 +115,23 @@ int vegas_set_table(vegas_ctx* ctx, const double* values, int n);
  *   integral = S1/n, error = sqrt(max(0,(S2/n - I^2)/(n-1))); hist (may be NULL) receives dim*nbins
  *   doubles, row-major [k][i].  The histogram also stays on the device for vegas_refine.
  * On success the iteration counter increments by one.  Non-finite results are returned as they are.
- * Errors: VEGAS_EINVAL (n_events < 2, events_per_launch == 0, NULL integral/error), VEGAS_ECUDA. */
+ * An iteration cut into 16 or more launches is captured once per (n_events, events_per_launch, seed, launch shape)
+ * into a CUDA graph and replayed (vegas_use_cuda_graph(ctx, 0) turns that off): at small batches the host's launch
+ * rate is otherwise the floor.  An iteration may have at most 2^20 launches.
+ * Errors: VEGAS_EINVAL (n_events < 2, events_per_launch == 0 or so small that the iteration would need more than
+ * 2^20 launches, NULL integral/error), VEGAS_ECUDA. */
 int vegas_iterate(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
                   double* integral, double* error, double* hist);
 
 /* Grid refinement (S7) from the histogram of the last vegas_iterate: 3-point smoothing, damping
  * ((1-r)/ln(1/r))^alpha, rebinning to equal damped weight; rebuilds the mapping table; clears H.
- * Errors: VEGAS_EINVAL (alpha < 0 or NaN), VEGAS_ESTATE (no histogram), VEGAS_EGRID (new edges not
- * strictly increasing: grid unchanged), VEGAS_ECUDA. */
+ * All-or-nothing over the dimensions: if any dimension's new edges are not strictly increasing the call returns
+ * VEGAS_EGRID and the grid, the table AND the histogram stay as they were, so the caller may refine again (for
+ * instance with another alpha); after a successful refinement the histogram is consumed (VEGAS_ESTATE until the
+ * next vegas_iterate).  vegas_set_grid and vegas_reset also drop the histogram (it was sampled through another grid).
+ * If an earlier vegas_refine_enqueue was rejected and not yet collected, this call still refines and then reports
+ * that rejection as VEGAS_EGRID (last_error says which).
+ * Errors: VEGAS_EINVAL (alpha < 0 or NaN), VEGAS_ESTATE (no histogram), VEGAS_EGRID, VEGAS_ECUDA. */
 int vegas_refine(vegas_ctx* ctx, double alpha);
 
 /* Asynchronous form of vegas_refine: enqueue only (no host synchronisation); the outcome of all refinements
@@ -157,7 +168,8 @@ int vegas_debug_events(vegas_ctx* ctx, uint64_t first_event, uint32_t count, uin
                        double* x, double* jac, double* f, double* wf, int32_t* pass);
 
 /* S1, S2 of the last vegas_iterate and the device time of everything it enqueued (CUDA events on the
- * context's stream: all launches + finalize, excluding the result copy).  Any pointer may be NULL.
+ * context's stream: all launches + finalize, excluding the result copy).  After a graph-replayed
+ * vegas_run_integration kernel_ms is that run's average device time per step.  Any pointer may be NULL.
  * VEGAS_ESTATE before the first iterate. */
 int vegas_last_sums(const vegas_ctx* ctx, double* S1, double* S2, double* kernel_ms);
 
@@ -167,7 +179,34 @@ int vegas_last_sums(const vegas_ctx* ctx, double* S1, double* S2, double* kernel
  * call enqueued. */
 int vegas_iterate_enqueue(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
                           int* n_kernel_launches);
-int vegas_iterate_collect(vegas_ctx* ctx, double* integral, double* error, double* hist);
+int vegas_iterate_collect(vegas_ctx* ctx, double* integral, double* error, double* hist);   /* hist after a successful
+                                                      * vegas_refine: VEGAS_ESTATE (it was consumed) */
+
+/* NEXT-2, multi-GPU sharding ("ensure that all GPUs ... receive a share"):
+ * events are counter-indexed, so GPU g of G runs the events [first, first + count) of an iteration of n_total events
+ * and the only exchange is one sum over the GPUs of the unreduced partials.
+ *   vegas_iterate_shard_enqueue  S1-S5 for [first, first + count) (count may be 0), cut into launches like
+ *                                vegas_iterate; leaves the shard's partial sums in the partials region; increments
+ *                                the iteration counter; no host synchronisation.
+ *   vegas_partials               device pointer and length (doubles) of that region, contiguous and 256-byte
+ *                                aligned: {S1.hi, S1.lo, S2.hi, S2.lo, npass, 0, 0, 0, H[dim][nbins]} -- S1 = S1.hi +
+ *                                S1.lo (a compensated pair), npass as a double.  The harness adds the regions of
+ *                                all GPUs in place (torch.distributed.all_reduce(SUM) on a tensor view: one call of
+ *                                8 + dim*nbins doubles per iteration, NCCL on GPUs), on the context's stream.
+ *   vegas_finalize_enqueue       S6 from the (summed) region: I, sigma for n_total events; afterwards
+ *                                vegas_iterate_collect / vegas_last_sums / vegas_last_npass / vegas_refine work as
+ *                                after vegas_iterate, and every GPU refines to the identical grid.
+ * Errors: VEGAS_EINVAL (range outside [0, n_total), n_total < 2, events_per_launch == 0), VEGAS_ESTATE (finalize
+ * without a shard; collect/refine between shard and finalize), VEGAS_ECUDA. */
+int vegas_iterate_shard_enqueue(vegas_ctx* ctx, uint64_t n_total, uint64_t first, uint64_t count,
+                                uint64_t events_per_launch, uint64_t seed, int* n_kernel_launches);
+int vegas_partials(const vegas_ctx* ctx, void** dev_partials, size_t* n_doubles);
+int vegas_finalize_enqueue(vegas_ctx* ctx, uint64_t n_total);
+
+/* Test hook: load H (dim*nbins doubles >= 0, row-major [k][i], host) as if a vegas_iterate had produced it, so that
+ * hand-made histograms reach the refinement kernel (the independent pins of S7).  Synchronises.
+ * Errors: VEGAS_EINVAL (NULL, a negative or NaN cell), VEGAS_ECUDA. */
+int vegas_set_histogram(vegas_ctx* ctx, const double* hist);
 
 /* Launch-shape tuning knobs of the iterate kernel (the batch-size / occupancy study):
  * CTAs per SM and threads per CTA (0 = the kernel instance's default, 1 x 1024 for the instances tuned to the
@@ -205,9 +244,11 @@ int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
  * combination is host arithmetic over n_iter numbers (vegas_combine_iterations, callable on its own, no GPU).
  * By default the whole step {memset, launches, finalize, refine, commit} is captured once into a CUDA graph and
  * replayed (the iteration counter then lives in device memory and the per-iteration (I, sigma) are logged on the
- * device; one host synchronisation per 64 iterations; iter_kernel_ms receives the average device time of a step,
- * refinement included).  vegas_use_cuda_graph(ctx, 0) selects the plain loop of blocking calls (per-iteration
- * times, refinement excluded).  Both give the same numbers.
+ * device together with a device time stamp; one host synchronisation per 64 iterations; iter_kernel_ms[i] is the
+ * device time from the end of iteration i-1 -- for the first one, from the start of the run -- to the end of
+ * iteration i, i.e. refinement i-1 + iteration i, read from %globaltimer).  vegas_use_cuda_graph(ctx, 0) selects the
+ * plain loop of blocking calls (per-iteration times from CUDA events, refinement excluded) and also keeps
+ * vegas_iterate from replaying graphs of many-launch iterations.  Both give the same numbers.
  * Errors: VEGAS_EINVAL (n_iter < 1, n_warmup < 0, NULL mean/error, iterate's argument errors), VEGAS_ECUDA. */
 int vegas_use_cuda_graph(vegas_ctx* ctx, int enable);
 int vegas_run_integration(vegas_ctx* ctx, int n_iter, int n_warmup, uint64_t n_events, uint64_t events_per_launch,

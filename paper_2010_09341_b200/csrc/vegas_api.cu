@@ -27,6 +27,11 @@ constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most re
 constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
 constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the iterate grid (CTAs)
 constexpr int kMaxSlots = kLanes * kLaneSlots;
+constexpr size_t kStaticSmemReserve = 1024;   // the opt-in shared-memory limit covers static + dynamic: room for the kernels' few static words
+constexpr int kPartHeader = 8;          // doubles in front of H: S1.hi, S1.lo, S2.hi, S2.lo, npass, pad[3] (vegas_partials)
+constexpr uint32_t kDebugChunk = 4096;  // events per pass of vegas_debug_events through the workspace's scratch region
+constexpr uint64_t kMaxLaunches = uint64_t(1) << 20;   // sanity bound on the launches of one iteration
+constexpr uint64_t kGraphMinLaunches = 16;   // vegas_iterate replays a captured graph from this many launches on
 constexpr double kPi = 0x1.921fb54442d18p+1;   // fl64(pi)
 
 thread_local char g_err[4096] = "";
@@ -51,7 +56,8 @@ size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // ---- device workspace layout (all offsets 256-byte aligned) -------------------------------------
 struct Layout {
-    size_t edges, new_edges, table, zero_begin, hist, slots, npass, zero_end, result, flags, status, dev_iter, ring, idata, total;
+    size_t edges, new_edges, table, zero_begin, part, hist, slots, npass, zero_end, result, flags, status, dev_iter, ring, idata,
+        scratch, total;
 };
 
 Layout make_layout(int dim, int nbins)
@@ -62,17 +68,20 @@ Layout make_layout(int dim, int nbins)
     L.edges = o;      o = align_up(o + nedges * 8, 256);
     L.new_edges = o;  o = align_up(o + nedges * 8, 256);
     L.table = o;      o = align_up(o + cells * 16, 256);
-    L.zero_begin = o;                                   // [hist | slots | npass] is cleared by one memset
-    L.hist = o;       o = align_up(o + cells * 8, 256);
+    L.zero_begin = o;                                   // [partials header | hist | slots | npass] is cleared by one memset
+    L.part = o;                                         // the unreduced partials of one iteration, contiguous (NEXT-2):
+    L.hist = o + kPartHeader * 8;                       // 8-double header, then H[dim][nbins]
+    o = align_up(L.hist + cells * 8, 256);
     L.slots = o;      o = align_up(o + static_cast<size_t>(kMaxSlots) * 32, 256);
     L.npass = o;      o = align_up(o + 8, 256);
     L.zero_end = o;
     L.result = o;     o = align_up(o + 64, 256);
     L.flags = o;      o = align_up(o + kMaxDim * 4, 256);
-    L.status = o;     o = align_up(o + 8, 256);                    // refine status word + ticket counter
+    L.status = o;     o = align_up(o + 16, 256);                   // refine: rejected count, ticket counter, latest outcome
     L.dev_iter = o;   o = align_up(o + 4, 256);                    // iteration counter of CUDA-graph replays
-    L.ring = o;       o = align_up(o + static_cast<size_t>(kRing) * 16, 256);   // their (I, sigma) log
+    L.ring = o;       o = align_up(o + (static_cast<size_t>(kRing) * 3 + 1) * 8, 256);   // their (I, sigma, time stamp) log + start stamp
     L.idata = o;      o = align_up(o + static_cast<size_t>(kMaxTable) * 8, 256);     // integrand data (vegas_set_table)
+    L.scratch = o;    o = align_up(o + static_cast<size_t>(kDebugChunk) * (static_cast<size_t>(dim) * 12 + 32), 256);   // vegas_debug_events
     L.total = o;
     return L;
 }
@@ -256,6 +265,13 @@ struct vegas_ctx {
     cudaEvent_t lane_done[kLanes], fork;
     uint64_t last_n;
     int last_launches;
+    bool hist_consumed;              // the latest refinement took the histogram and no iteration ran since: a rejected
+                                     // refinement gives it back (grid and H unchanged, DESIGN.md section 2 S7)
+    bool last_graph;                 // the latest iteration(s) ran as graph replays of whole steps: no per-iteration events
+    double last_graph_ms;            // their average device time per step
+    bool shard_pending;              // vegas_iterate_shard_enqueue ran and vegas_finalize_enqueue has not yet
+    cudaGraphExec_t igexec;          // captured {memset, launches} of one many-launch iteration (vegas_iterate) for the key below
+    uint64_t ig_n, ig_first, ig_count, ig_epl, ig_seed; int ig_threads, ig_ctas, ig_rshift, ig_shard, ig_launches; const Instance* ig_inst;
 };
 
 namespace {
@@ -332,7 +348,7 @@ int pick_rshift(const vegas_ctx* c, const Instance* in, int ctas, int threads)
     const size_t per_sm = 228u * 1024u;
     for (int rs = 5; rs >= 0; --rs) {
         const size_t need = iterate_smem_bytes(c, in, rs, threads) + 1024;   // 1 KB reserved per CTA
-        if (need * ctas <= per_sm && need - 1024 <= static_cast<size_t>(c->smem_optin)) return rs;
+        if (need * ctas <= per_sm && need <= static_cast<size_t>(c->smem_optin)) return rs;
     }
     return -1;
 }
@@ -352,8 +368,10 @@ int apply_shape(vegas_ctx* c, int ctas, int threads, int rshift)
     else if (rshift < 0) rshift = pick_rshift(c, in, ctas, threads);
     if (rshift < 0 || rshift > 5) return fail(VEGAS_EINVAL, "histogram of %d x %d cells does not fit in shared memory with %d CTAs/SM", c->dim, c->nbins, ctas);
     const size_t smem = iterate_smem_bytes(c, in, rshift, threads);
-    if (smem > static_cast<size_t>(c->smem_optin)) return fail(VEGAS_EINVAL, "needs %zu bytes of shared memory per CTA, device allows %d", smem, c->smem_optin);
-    CUDA_TRY(inst_set_smem(in, static_cast<int>(smem)));
+    if (smem > static_cast<size_t>(c->smem_optin) - kStaticSmemReserve) return fail(VEGAS_EINVAL, "needs %zu bytes of shared memory per CTA, device allows %d", smem, c->smem_optin - static_cast<int>(kStaticSmemReserve));
+    // cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel function, not to this context: contexts that
+    // share a generic instance with different shapes must not lower each other's limit, so it is always the device maximum
+    CUDA_TRY(inst_set_smem(in, c->smem_optin - static_cast<int>(kStaticSmemReserve)));
     int occ = 0;
     CUDA_TRY(inst_occupancy(in, &occ, threads, smem));
     if (occ < 1) return fail(VEGAS_EINVAL, "launch shape (%d threads, %zu B smem) cannot run", threads, smem);
@@ -368,6 +386,7 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
 {
     a.table = c->ws + c->L.table;
     a.hist = reinterpret_cast<double*>(c->ws + c->L.hist);
+    a.partials = reinterpret_cast<double*>(c->ws + c->L.part);
     a.slots = reinterpret_cast<double*>(c->ws + c->L.slots);
     a.npass = reinterpret_cast<unsigned long long*>(c->ws + c->L.npass);
     a.e_lo_first = static_cast<uint32_t>(first);
@@ -479,6 +498,7 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     for (int i = 0; i < kEvPool; ++i) { c->evA[i] = nullptr; c->evB[i] = nullptr; }
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0; c->rt_lib = nullptr; c->rt_inst = nullptr;
+    c->hist_consumed = false; c->last_graph = false; c->last_graph_ms = 0.0; c->shard_pending = false; c->igexec = nullptr;
     c->n_user_params = n_params;
     int rc = setup_integrand(c, params);
     if (rc != VEGAS_OK) { delete c; return rc; }
@@ -488,7 +508,8 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     cudaDeviceProp prop;
     if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess)
         return cleanup(fail(VEGAS_ECUDA, "cudaGetDeviceProperties failed"));
-    if (prop.major < 10) return cleanup(fail(VEGAS_ECUDA, "device sm_%d%d: this library is built for sm_100a only", prop.major, prop.minor));
+    if (prop.major != 10 || prop.minor != 0)             // the library carries sm_100a SASS only (no PTX)
+        return cleanup(fail(VEGAS_EUNSUPPORTED, "device sm_%d%d: this library is built for sm_100a (B200) only", prop.major, prop.minor));
     c->sm_count = prop.multiProcessorCount;
     c->smem_optin = static_cast<int>(prop.sharedMemPerBlockOptin);
     int khz = 0;
@@ -496,7 +517,7 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     c->sm_clock_khz = khz;
     if (cudaHostAlloc(reinterpret_cast<void**>(&c->h_result), (8 + static_cast<size_t>(dim) * nbins) * sizeof(double), cudaHostAllocDefault) != cudaSuccess ||
         cudaHostAlloc(reinterpret_cast<void**>(&c->h_status), 64, cudaHostAllocDefault) != cudaSuccess ||
-        cudaHostAlloc(reinterpret_cast<void**>(&c->h_ring), kRing * 16, cudaHostAllocDefault) != cudaSuccess ||
+        cudaHostAlloc(reinterpret_cast<void**>(&c->h_ring), (kRing * 3 + 1) * 8, cudaHostAllocDefault) != cudaSuccess ||
         cudaEventCreate(&c->run_ev0) != cudaSuccess || cudaEventCreate(&c->run_ev1) != cudaSuccess ||
         cudaStreamCreateWithFlags(&c->gstream, cudaStreamNonBlocking) != cudaSuccess ||
         !create_event_pool(c) ||
@@ -563,6 +584,7 @@ void vegas_destroy(vegas_ctx* c)
         if (c->evB[i]) cudaEventDestroy(c->evB[i]);
     }
     if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->igexec) cudaGraphExecDestroy(c->igexec);
     if (c->rt_lib) cudaLibraryUnload(c->rt_lib);
     delete c->rt_inst;
     if (c->fork) cudaEventDestroy(c->fork);
@@ -609,39 +631,143 @@ int vegas_device_info(const vegas_ctx* c, int* sm_count, int* sm_clock_khz)
     return VEGAS_OK;
 }
 
-static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
-                             int* n_kernel_launches, bool graph_mode);
+// How the kernels of one iteration get their Philox iteration word and what the last CTA does with the sums.
+enum IterMode {
+    kPlain = 0,        // counter word in the kernel arguments; S6 in the last CTA
+    kGraphStep = 1,    // captured whole step (vegas_run_integration): counter in device memory, S6 logs (I, sigma) to the
+                       // ring and advances the counter
+    kGraphIter = 2     // captured iteration (vegas_iterate with many launches): counter in device memory, written by the
+                       // host before every replay
+};
+
+static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
+                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard);
+static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
+                          uint64_t seed, int* n_kernel_launches, bool shard);
 
 int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
                           int* n_kernel_launches)
 {
-    return enqueue_iteration(c, n_events, events_per_launch, seed, n_kernel_launches, false);
+    return iterate_common(c, n_events, 0, n_events, events_per_launch, seed, n_kernel_launches, false);
 }
 
-// graph_mode: called between cudaStreamBeginCapture / EndCapture.  The iteration counter is read from device
-// memory (finalize advances it and logs (I, sigma) to the ring), no timing events are recorded, and the host-side
-// bookkeeping (iteration counter, event pool) is left to the caller.
-static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
-                             int* n_kernel_launches, bool graph_mode)
+int vegas_iterate_shard_enqueue(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count,
+                                uint64_t events_per_launch, uint64_t seed, int* n_kernel_launches)
+{
+    return iterate_common(c, n_total, first, count, events_per_launch, seed, n_kernel_launches, true);
+}
+
+static int check_iteration_args(const vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t epl,
+                                uint64_t* n_launches)
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
-    if (n_events < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
+    if (n_total < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
     if (c->integrand_id == VEGAS_LO_2TO2_TAB && !c->ic.tab) return fail(VEGAS_ESTATE, "lo_2to2_tab needs vegas_set_table first");
-    if (events_per_launch == 0) return fail(VEGAS_EINVAL, "events_per_launch must be > 0");
-    if (n_events > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
-    const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
+    if (epl == 0) return fail(VEGAS_EINVAL, "events_per_launch must be > 0");
+    if (n_total > (uint64_t(1) << 53)) return fail(VEGAS_EINVAL, "n_events must be <= 2^53");
+    if (first > n_total || count > n_total - first) return fail(VEGAS_EINVAL, "shard [first, first + count) must lie inside [0, n_total)");
+    const uint64_t e = epl < (uint64_t(1) << 31) ? epl : (uint64_t(1) << 31);
+    // launches: ceil(count / epl) plus at most one more per multiple of 2^32 inside the range (a launch never straddles one)
+    const uint64_t bound = (count + e - 1) / e + (count >> 32) + 2;
+    if (bound > kMaxLaunches)
+        return fail(VEGAS_EINVAL, "%llu events in launches of %llu: more than %llu launches for one iteration (raise events_per_launch)",
+                    static_cast<unsigned long long>(count), static_cast<unsigned long long>(e), static_cast<unsigned long long>(kMaxLaunches));
+    if (n_launches) *n_launches = bound;
+    return VEGAS_OK;
+}
+
+__global__ void set_u32_kernel(uint32_t* p, uint32_t v) { *p = v; }
+
+// Capture {memset, all launches} of one iteration with this geometry into a CUDA graph (kept until the key changes).
+static int ensure_iter_graph(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t epl, uint64_t seed,
+                             bool shard, int* launches)
+{
+    if (c->igexec && c->ig_n == n_total && c->ig_first == first && c->ig_count == count && c->ig_epl == epl &&
+        c->ig_seed == seed && c->ig_shard == (shard ? 1 : 0) && c->ig_threads == c->threads && c->ig_ctas == c->ctas_per_sm &&
+        c->ig_rshift == c->rshift && c->ig_inst == c->inst) {
+        if (launches) *launches = c->ig_launches;
+        return VEGAS_OK;
+    }
+    if (c->igexec) { cudaGraphExecDestroy(c->igexec); c->igexec = nullptr; }
+    cudaStream_t user = c->stream;
+    c->stream = c->gstream;                              // the caller's stream may be the legacy default stream (no capture)
+    cudaError_t e = cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeRelaxed);
+    if (e != cudaSuccess) { c->stream = user; return fail(VEGAS_ECUDA, "cudaStreamBeginCapture failed: %s", cudaGetErrorString(e)); }
+    int nl = 0;
+    const int rc = enqueue_iteration(c, n_total, first, count, epl, seed, &nl, kGraphIter, shard);
+    cudaGraph_t graph = nullptr;
+    e = cudaStreamEndCapture(c->gstream, &graph);       // always leave capture mode
+    c->stream = user;
+    if (rc != VEGAS_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(VEGAS_ECUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
+    const cudaError_t e2 = cudaGraphInstantiate(&c->igexec, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e2 != cudaSuccess) { c->igexec = nullptr; return fail(VEGAS_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    c->ig_n = n_total; c->ig_first = first; c->ig_count = count; c->ig_epl = epl; c->ig_seed = seed; c->ig_shard = shard ? 1 : 0;
+    c->ig_threads = c->threads; c->ig_ctas = c->ctas_per_sm; c->ig_rshift = c->rshift; c->ig_inst = c->inst;
+    c->ig_launches = nl;
+    if (launches) *launches = nl;
+    return VEGAS_OK;
+}
+
+// One iteration (or one shard of it) on the context's stream, bracketed by the event pair of the pool, with the
+// host-side bookkeeping.  Iterations cut into many launches replay a captured graph (vegas_use_cuda_graph): the
+// host's launch rate (2-2.5 us per cudaLaunchKernel) is otherwise the floor of small batches.
+static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
+                          uint64_t seed, int* n_kernel_launches, bool shard)
+{
+    uint64_t bound = 0;
+    int rc = check_iteration_args(c, n_total, first, count, events_per_launch, &bound);
+    if (rc != VEGAS_OK) return rc;
     const int evi = static_cast<int>(c->n_enqueued % kEvPool);
-    if (!graph_mode) CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
+    int launches = 0;
+    const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
+    if (c->use_graph && (count + epl - 1) / epl >= kGraphMinLaunches) {
+        rc = ensure_iter_graph(c, n_total, first, count, events_per_launch, seed, shard, &launches);
+        if (rc != VEGAS_OK) return rc;
+        CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
+        set_u32_kernel<<<1, 1, 0, c->stream>>>(reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter), c->iteration);
+        CUDA_TRY(cudaGraphLaunch(c->igexec, c->stream));
+    } else {
+        CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
+        rc = enqueue_iteration(c, n_total, first, count, events_per_launch, seed, &launches, kPlain, shard);
+        if (rc != VEGAS_OK) return rc;
+    }
+    CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
+    c->n_enqueued += 1;
+    c->iteration += 1;
+    c->have_hist = !shard;                               // a shard's H is partial until the all-reduce + vegas_finalize_enqueue
+    c->have_sums = !shard;
+    c->shard_pending = shard;
+    c->hist_consumed = false;
+    c->last_graph = false;
+    c->last_n = n_total;
+    c->last_launches = launches;
+    if (n_kernel_launches) *n_kernel_launches = launches;
+    return VEGAS_OK;
+}
+
+// Enqueue {memset, launches} of the events [first, first + count) of an iteration of n_total events.  Pure enqueue: no
+// timing events, no bookkeeping (iterate_common / the graph captures do that).
+static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
+                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard)
+{
+    uint64_t bound = 0;
+    const int rc0 = check_iteration_args(c, n_total, first, count, events_per_launch, &bound);
+    if (rc0 != VEGAS_OK) return rc0;
+    const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
     CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    if (n_kernel_launches) *n_kernel_launches = 0;
+    if (count == 0) return VEGAS_OK;                     // an empty shard contributes zeros
     IterArgs a;
     fill_args(c, seed, 0, 0, a);
-    if (graph_mode) a.iter_ptr = reinterpret_cast<const uint32_t*>(c->ws + c->L.dev_iter);
+    if (mode != kPlain) a.iter_ptr = reinterpret_cast<const uint32_t*>(c->ws + c->L.dev_iter);
     const int max_grid = c->ctas_per_sm * c->sm_count;
     // Launches of one iteration are independent (global event index; the histogram and the pass counter are
     // accumulated with global reductions; each lane has its own slot region), so when an iteration is cut into
     // several launches they are dealt round-robin to kLanes internal streams forked from the caller's stream:
     // launches that do not fill the GPU overlap, and every launch's prologue/flush overlaps its neighbours'.
-    const uint64_t n_launches = (n_events + epl - 1) / epl;
+    const uint64_t n_launches = (count + epl - 1) / epl;
     const int lanes = n_launches > 1 ? kLanes : 1;
     // several launches in flight: each takes a fraction of the SMs, so that one launch's prologue / flush overlaps
     // its neighbours' event loops (a CTA of a tuned instance fills an SM's shared memory: full-size grids cannot
@@ -654,48 +780,53 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
     }
     double* slots0 = reinterpret_cast<double*>(c->ws + c->L.slots);
-    // launch geometry of the whole iteration first: S6 runs in the CTA that finishes last, so every launch must
-    // know how many CTAs there are in total and how many slots each stream-lane region uses
-    auto launch_count = [&](uint64_t done) {
-        uint64_t cnt = n_events - done;
+    // launch geometry of the whole iteration first: the sums are folded in the CTA that finishes last, so every launch
+    // must know how many CTAs there are in total and how many slots each stream-lane region uses
+    const uint64_t last = first + count;
+    auto launch_count = [&](uint64_t at) {
+        uint64_t cnt = last - at;
         if (cnt > epl) cnt = epl;
-        const uint64_t to_wrap = (uint64_t(1) << 32) - (done & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
+        const uint64_t to_wrap = (uint64_t(1) << 32) - (at & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
         return cnt > to_wrap ? to_wrap : cnt;
     };
+    // a CTA's prologue and flush (zero and sum R replicas of d*N cells) cost as much as several grid-strides of events:
+    // when many small launches share the GPU each gets fewer CTAs with at least kMinStrides events per thread
+    const uint64_t kMinStrides = n_launches >= 8 ? 4 : 1;
     auto launch_grid = [&](uint64_t cnt) {
-        const uint64_t want = (cnt + c->threads - 1) / c->threads;
+        uint64_t want = (cnt + static_cast<uint64_t>(c->threads) * kMinStrides - 1) / (static_cast<uint64_t>(c->threads) * kMinStrides);
+        if (want < 1) want = 1;
         return want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
     };
     uint64_t total_ctas = 0;
     int used_grid = 0;
-    for (uint64_t done = 0; done < n_events;) {
-        const uint64_t cnt = launch_count(done);
+    for (uint64_t at = first; at < last;) {
+        const uint64_t cnt = launch_count(at);
         const int grid = launch_grid(cnt);
         total_ctas += static_cast<uint64_t>(grid);
         if (grid > used_grid) used_grid = grid;
-        done += cnt;
+        at += cnt;
     }
     if (total_ctas > 0xFFFFFFFFull) return fail(VEGAS_EINVAL, "too many launches for one iteration (raise events_per_launch)");
     a.ticket = reinterpret_cast<unsigned int*>(c->ws + c->L.npass) + 4;   // inside the region cleared by the memset
     a.total_ctas = static_cast<unsigned int>(total_ctas);
     a.slots0 = slots0;
     a.fin_lanes = lanes; a.fin_stride = kLaneSlots; a.fin_used = used_grid;
-    a.n_events = n_events;
+    a.n_events = shard ? 0ull : n_total;
     a.result = reinterpret_cast<double*>(c->ws + c->L.result);
-    a.dev_iter = graph_mode ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr;
-    a.ring = graph_mode ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr;
+    a.dev_iter = (mode == kGraphStep) ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr;
+    a.ring = (mode == kGraphStep) ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr;
     a.ring_len = kRing;
     int launches = 0;
-    for (uint64_t done = 0; done < n_events;) {
-        const uint64_t cnt = launch_count(done);
-        a.e_lo_first = static_cast<uint32_t>(done);
-        a.e_hi = static_cast<uint32_t>(done >> 32);
+    for (uint64_t at = first; at < last;) {
+        const uint64_t cnt = launch_count(at);
+        a.e_lo_first = static_cast<uint32_t>(at);
+        a.e_hi = static_cast<uint32_t>(at >> 32);
         a.count = static_cast<uint32_t>(cnt);
         const int grid = launch_grid(cnt);
         const int ln = launches % lanes;
         a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
         CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
-        done += cnt;
+        at += cnt;
         ++launches;
     }
     if (lanes > 1) {
@@ -706,17 +837,29 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_events, uint64_t events_pe
     }
     CUDA_TRY(cudaGetLastError());
     if (n_kernel_launches) *n_kernel_launches = launches;
-    c->have_hist = true;
-    c->last_launches = launches;
-    if (graph_mode) return VEGAS_OK;
-    CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
-    c->n_enqueued += 1;
-    c->iteration += 1;
+    return VEGAS_OK;
+}
+
+int vegas_partials(const vegas_ctx* c, void** dev_partials, size_t* n_doubles)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (dev_partials) *dev_partials = c->ws + c->L.part;
+    if (n_doubles) *n_doubles = kPartHeader + static_cast<size_t>(c->dim) * c->nbins;
+    return VEGAS_OK;
+}
+
+int vegas_finalize_enqueue(vegas_ctx* c, uint64_t n_total)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (n_total < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
+    if (!c->shard_pending) return fail(VEGAS_ESTATE, "vegas_finalize_enqueue follows vegas_iterate_shard_enqueue");
+    finalize_kernel<<<1, 32, 0, c->stream>>>(reinterpret_cast<const double*>(c->ws + c->L.part), n_total,
+                                             reinterpret_cast<double*>(c->ws + c->L.result));
+    CUDA_TRY(cudaGetLastError());
+    c->shard_pending = false;
     c->have_hist = true;
     c->have_sums = true;
-    c->last_n = n_events;
-    c->last_launches = launches;
-    if (n_kernel_launches) *n_kernel_launches = launches;
+    c->last_n = n_total;
     return VEGAS_OK;
 }
 
@@ -724,7 +867,8 @@ int vegas_iterate_collect(vegas_ctx* c, double* integral, double* error, double*
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (!integral || !error) return fail(VEGAS_EINVAL, "integral and error are required");
-    if (!c->have_sums) return fail(VEGAS_ESTATE, "no iteration has been enqueued");
+    if (!c->have_sums) return fail(VEGAS_ESTATE, "no finished iteration (a shard needs vegas_finalize_enqueue first)");
+    if (hist && !c->have_hist) return fail(VEGAS_ESTATE, "the histogram of the last iteration was consumed by vegas_refine");
     const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
     CUDA_TRY(cudaMemcpyAsync(c->h_result, c->ws + c->L.result, 64, cudaMemcpyDeviceToHost, c->stream));
     if (hist) CUDA_TRY(cudaMemcpyAsync(c->h_result + 8, c->ws + c->L.hist, cells * 8, cudaMemcpyDeviceToHost, c->stream));
@@ -754,10 +898,14 @@ int vegas_last_sums(const vegas_ctx* c, double* S1, double* S2, double* kernel_m
     if (S1) *S1 = c->h_result[2];
     if (S2) *S2 = c->h_result[3];
     if (kernel_ms) {
-        float ms = 0.f;
-        const int evi = static_cast<int>((c->n_enqueued - 1) % kEvPool);
-        CUDA_TRY(cudaEventElapsedTime(&ms, c->evA[evi], c->evB[evi]));
-        *kernel_ms = ms;
+        if (c->last_graph) *kernel_ms = c->last_graph_ms;        // graph-replayed steps: their average device time
+        else {
+            if (c->n_enqueued == 0) return fail(VEGAS_ESTATE, "no iteration has been timed yet");
+            float ms = 0.f;
+            const int evi = static_cast<int>((c->n_enqueued - 1) % kEvPool);
+            CUDA_TRY(cudaEventElapsedTime(&ms, c->evA[evi], c->evB[evi]));
+            *kernel_ms = ms;
+        }
     }
     return VEGAS_OK;
 }
@@ -772,24 +920,40 @@ int vegas_last_npass(const vegas_ctx* c, uint64_t* npass)
     return VEGAS_OK;
 }
 
+int vegas_set_histogram(vegas_ctx* c, const double* hist)
+{
+    if (!c || !hist) return fail(VEGAS_EINVAL, "NULL argument");
+    const size_t cells = static_cast<size_t>(c->dim) * c->nbins;
+    for (size_t i = 0; i < cells; ++i)
+        if (!(hist[i] >= 0.0)) return fail(VEGAS_EINVAL, "histogram cell %zu is negative or NaN", i);
+    CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.hist, hist, cells * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(cudaStreamSynchronize(c->stream));          // `hist` is pageable host memory owned by the caller
+    c->have_hist = true;
+    c->hist_consumed = false;
+    c->shard_pending = false;
+    return VEGAS_OK;
+}
+
 int vegas_refine_enqueue(vegas_ctx* c, double alpha)
 {
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
     if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
     const int N = c->nbins;
-    const size_t smem = (3 * static_cast<size_t>(N) + 1) * sizeof(double);
-    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem)));
+    const size_t smem = (5 * static_cast<size_t>(N) + 2) * sizeof(double);
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - static_cast<int>(kStaticSmemReserve)));
     double* edges = reinterpret_cast<double*>(c->ws + c->L.edges);
     double* new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);
     double* hist = reinterpret_cast<double*>(c->ws + c->L.hist);
     int* flags = reinterpret_cast<int*>(c->ws + c->L.flags);
     int* status = reinterpret_cast<int*>(c->ws + c->L.status);
-    refine_kernel<<<c->dim, 128, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags, c->dim, c->ws + c->L.table,
-                                                    c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status,
-                                                    reinterpret_cast<unsigned int*>(c->ws + c->L.status) + 1);
+    const int threads = N >= 96 ? 128 : (N + 31) / 32 * 32;
+    refine_kernel<<<c->dim, threads, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags, c->dim, c->ws + c->L.table,
+                                                        c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status,
+                                                        reinterpret_cast<unsigned int*>(c->ws + c->L.status) + 1);
     CUDA_TRY(cudaGetLastError());
     c->have_hist = false;
+    c->hist_consumed = true;
     c->refine_pending += 1;
     return VEGAS_OK;
 }
@@ -799,23 +963,30 @@ int vegas_refine_collect(vegas_ctx* c)
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (c->refine_pending == 0) return VEGAS_OK;
     int* status = reinterpret_cast<int*>(c->ws + c->L.status);
-    CUDA_TRY(cudaMemcpyAsync(c->h_status, status, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(cudaMemcpyAsync(c->h_status, status, 3 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CUDA_TRY(cudaMemsetAsync(status, 0, sizeof(int), c->stream));
     CUDA_TRY(cudaStreamSynchronize(c->stream));
     const int pending = c->refine_pending;
     c->refine_pending = 0;
+    // the latest refinement was rejected and nothing overwrote H since: the histogram is still there for another try
+    if (c->h_status[2] != 0 && c->hist_consumed) { c->have_hist = true; c->hist_consumed = false; }
     if (c->h_status[0] != 0)
-        return fail(VEGAS_EGRID, "refined edges were not strictly increasing in at least one of the last %d refinement(s); that grid was left unchanged", pending);
+        return fail(VEGAS_EGRID, "refined edges were not strictly increasing in %d of the last %d refinement(s); each of those left its grid and histogram unchanged", c->h_status[0], pending);
     return VEGAS_OK;
 }
 
 int vegas_refine(vegas_ctx* c, double alpha)
 {
-    int rc = vegas_refine_collect(c);                    // outcome of earlier asynchronous refinements first
-    if (rc != VEGAS_OK && rc != VEGAS_EGRID) return rc;
-    rc = vegas_refine_enqueue(c, alpha);
+    // the outcome of earlier asynchronous refinements first; a rejection among them is not dropped: it is reported
+    // by this call (after this refinement was attempted) unless this call fails for a reason of its own
+    const int rc0 = vegas_refine_collect(c);
+    if (rc0 != VEGAS_OK && rc0 != VEGAS_EGRID) return rc0;
+    int rc = vegas_refine_enqueue(c, alpha);
     if (rc != VEGAS_OK) return rc;
-    return vegas_refine_collect(c);
+    rc = vegas_refine_collect(c);
+    if (rc == VEGAS_OK && rc0 == VEGAS_EGRID)
+        return fail(VEGAS_EGRID, "this refinement was applied, but an earlier asynchronous refinement (vegas_refine_enqueue) had been rejected: its edges were not strictly increasing and it left its grid unchanged");
+    return rc;
 }
 
 int vegas_iteration_kernel_ms(const vegas_ctx* c, int back, double* kernel_ms)
@@ -853,6 +1024,8 @@ int vegas_tune_events_per_launch(vegas_ctx* c, uint64_t n_events, uint64_t seed,
     c->iteration = it0;
     c->have_hist = false;
     c->have_sums = false;
+    c->hist_consumed = false;
+    c->shard_pending = false;
     return rc;
 }
 
@@ -897,8 +1070,8 @@ static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint
         return VEGAS_OK;
     if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
     CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
-    int rc = enqueue_iteration(c, n_events, epl, seed, nullptr, true);
-    if (rc == VEGAS_OK) rc = vegas_refine_enqueue(c, alpha);
+    int rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false);
+    if (rc == VEGAS_OK) { c->have_hist = true; rc = vegas_refine_enqueue(c, alpha); }
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);     // always leave capture mode
     c->refine_pending = 0;
@@ -915,10 +1088,10 @@ static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint
 // `total` replays of the captured step; (I, sigma) of every iteration into I[], sg[]; average device time per
 // iteration into *avg_ms.  One host synchronisation per kRing iterations.
 static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
-                              double* I, double* sg, double* avg_ms);
+                              double* I, double* sg, double* iter_ms);
 
 static int run_steps_graph(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
-                           double* I, double* sg, double* avg_ms)
+                           double* I, double* sg, double* iter_ms)
 {
     int rc = vegas_refine_collect(c);
     if (rc != VEGAS_OK && rc != VEGAS_EGRID) return rc;
@@ -927,14 +1100,14 @@ static int run_steps_graph(vegas_ctx* c, int total, uint64_t n_events, uint64_t 
     CUDA_TRY(cudaEventRecord(c->fork, user));
     CUDA_TRY(cudaStreamWaitEvent(c->gstream, c->fork, 0));
     c->stream = c->gstream;
-    rc = run_steps_graph_on(c, total, n_events, epl, seed, alpha, I, sg, avg_ms);
+    rc = run_steps_graph_on(c, total, n_events, epl, seed, alpha, I, sg, iter_ms);
     c->stream = user;
     if (cudaEventRecord(c->fork, c->gstream) == cudaSuccess) cudaStreamWaitEvent(user, c->fork, 0);
     return rc;
 }
 
 static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha,
-                              double* I, double* sg, double* avg_ms)
+                              double* I, double* sg, double* iter_ms)
 {
     int rc;
     rc = ensure_step_graph(c, n_events, epl, seed, alpha);
@@ -942,26 +1115,37 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     uint32_t* h_it = reinterpret_cast<uint32_t*>(c->h_status) + 4;
     *h_it = c->iteration;
     CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.dev_iter, h_it, 4, cudaMemcpyHostToDevice, c->stream));
+    double* ring = reinterpret_cast<double*>(c->ws + c->L.ring);
+    stamp_kernel<<<1, 1, 0, c->stream>>>(ring + 3 * kRing);
     CUDA_TRY(cudaEventRecord(c->run_ev0, c->stream));
+    auto stamp_of = [](double v) { long long t; std::memcpy(&t, &v, 8); return t; };
+    long long t_prev = 0;
     for (int done = 0; done < total;) {
         const int chunk = (total - done < kRing) ? total - done : kRing;
         for (int i = 0; i < chunk; ++i) CUDA_TRY(cudaGraphLaunch(c->gexec, c->stream));
         if (done + chunk == total) CUDA_TRY(cudaEventRecord(c->run_ev1, c->stream));
-        CUDA_TRY(cudaMemcpyAsync(c->h_ring, c->ws + c->L.ring, kRing * 16, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(cudaMemcpyAsync(c->h_ring, ring, (kRing * 3 + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(cudaStreamSynchronize(c->stream));
+        if (done == 0) t_prev = stamp_of(c->h_ring[3 * kRing]);
         for (int i = 0; i < chunk; ++i) {
             const uint32_t it = c->iteration + static_cast<uint32_t>(done + i);
-            I[done + i] = c->h_ring[2 * (it % kRing) + 0];
-            sg[done + i] = c->h_ring[2 * (it % kRing) + 1];
+            I[done + i] = c->h_ring[3 * (it % kRing) + 0];
+            sg[done + i] = c->h_ring[3 * (it % kRing) + 1];
+            const long long t = stamp_of(c->h_ring[3 * (it % kRing) + 2]);
+            if (iter_ms) iter_ms[done + i] = static_cast<double>(t - t_prev) * 1e-6;
+            t_prev = t;
         }
         done += chunk;
     }
     float ms = 0.f;
     CUDA_TRY(cudaEventElapsedTime(&ms, c->run_ev0, c->run_ev1));
-    if (avg_ms) *avg_ms = static_cast<double>(ms) / total;
+    c->last_graph = true;
+    c->last_graph_ms = static_cast<double>(ms) / total;
     c->iteration += static_cast<uint32_t>(total);
     c->have_hist = false;                                // the last step refined
+    c->hist_consumed = true;
     c->have_sums = true;
+    c->shard_pending = false;
     c->last_n = n_events;
     c->refine_pending = total;
     rc = vegas_refine_collect(c);
@@ -978,6 +1162,7 @@ int vegas_set_table(vegas_ctx* c, const double* values, int n)
     c->ic.tab = reinterpret_cast<const double*>(c->ws + c->L.idata);
     c->ic.ntab = n;
     if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }   // captured kernel arguments are stale
+    if (c->igexec) { cudaGraphExecDestroy(c->igexec); c->igexec = nullptr; }
     return VEGAS_OK;
 }
 
@@ -1002,9 +1187,7 @@ int vegas_run_integration(vegas_ctx* c, int n_iter, int n_warmup, uint64_t n_eve
     int rc = VEGAS_OK;
     if (c->use_graph) {
         if (n_events < 2 || events_per_launch == 0) { std::free(I); return fail(VEGAS_EINVAL, "n_events >= 2 and events_per_launch > 0 required"); }
-        double avg = 0.0;
-        rc = run_steps_graph(c, total, n_events, events_per_launch, seed, alpha, I, sg, &avg);
-        if (rc == VEGAS_OK && iter_kernel_ms) for (int it = 0; it < total; ++it) iter_kernel_ms[it] = avg;
+        rc = run_steps_graph(c, total, n_events, events_per_launch, seed, alpha, I, sg, iter_kernel_ms);
     } else
     for (int it = 0; it < total && rc == VEGAS_OK; ++it) {
         rc = vegas_iterate(c, n_events, events_per_launch, seed, &I[it], &sg[it], nullptr);
@@ -1045,6 +1228,8 @@ int vegas_set_grid(vegas_ctx* c, const double* edges)
     const int rc = build_table(c, 0);
     if (rc != VEGAS_OK) return rc;
     CUDA_TRY(cudaStreamSynchronize(c->stream));
+    c->have_hist = false;                                // H was sampled through the old grid: it must not refine the new one
+    c->hist_consumed = false;
     return VEGAS_OK;
 }
 
@@ -1058,6 +1243,8 @@ int vegas_reset(vegas_ctx* c)
     c->iteration = 0;
     c->have_hist = false;
     c->have_sums = false;
+    c->hist_consumed = false;
+    c->shard_pending = false;
     return VEGAS_OK;
 }
 
@@ -1081,32 +1268,33 @@ int vegas_debug_events(vegas_ctx* c, uint64_t first_event, uint32_t count, uint6
     if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
     if (count == 0) return VEGAS_OK;
     if ((first_event & 0xFFFFFFFFull) + count > (uint64_t(1) << 32)) return fail(VEGAS_EINVAL, "range straddles a multiple of 2^32");
+    // kDebugChunk events at a time through the scratch region of the caller's workspace (the library allocates no
+    // device memory)
     const size_t d = static_cast<size_t>(c->dim);
-    const size_t b_bins = align_up(count * d * 4, 256), b_x = align_up(count * d * 8, 256), b_s = align_up(static_cast<size_t>(count) * 8, 256),
-                 b_p = align_up(static_cast<size_t>(count) * 4, 256);
-    unsigned char* tmp = nullptr;                        // temporary device buffer, freed before return
-    CUDA_TRY(cudaMalloc(reinterpret_cast<void**>(&tmp), b_bins + b_x + 3 * b_s + b_p));
-    int32_t* d_bins = reinterpret_cast<int32_t*>(tmp);
-    double* d_x = reinterpret_cast<double*>(tmp + b_bins);
-    double* d_jac = reinterpret_cast<double*>(tmp + b_bins + b_x);
-    double* d_f = reinterpret_cast<double*>(tmp + b_bins + b_x + b_s);
-    double* d_wf = reinterpret_cast<double*>(tmp + b_bins + b_x + 2 * b_s);
-    int32_t* d_pass = reinterpret_cast<int32_t*>(tmp + b_bins + b_x + 3 * b_s);
-    IterArgs a;
-    fill_args(c, seed, first_event, count, a);
-    cudaError_t e = inst_debug(c->inst, a, static_cast<int>((count + 127) / 128), 128, c->stream, d_bins, d_x, d_jac, d_f, d_wf, d_pass);
-    auto copy = [&](void* dst, const void* src, size_t n) {
-        if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToHost, c->stream);
-    };
-    copy(bins, d_bins, count * d * 4);
-    copy(x, d_x, count * d * 8);
-    copy(jac, d_jac, static_cast<size_t>(count) * 8);
-    copy(f, d_f, static_cast<size_t>(count) * 8);
-    copy(wf, d_wf, static_cast<size_t>(count) * 8);
-    copy(pass, d_pass, static_cast<size_t>(count) * 4);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    cudaFree(tmp);
-    if (e != cudaSuccess) return fail(VEGAS_ECUDA, "vegas_debug_events: %s", cudaGetErrorString(e));
+    unsigned char* tmp = c->ws + c->L.scratch;
+    double* d_x = reinterpret_cast<double*>(tmp);
+    double* d_jac = d_x + kDebugChunk * d;
+    double* d_f = d_jac + kDebugChunk;
+    double* d_wf = d_f + kDebugChunk;
+    int32_t* d_bins = reinterpret_cast<int32_t*>(d_wf + kDebugChunk);
+    int32_t* d_pass = d_bins + kDebugChunk * d;
+    for (uint32_t done = 0; done < count; done += kDebugChunk) {
+        const uint32_t n = (count - done < kDebugChunk) ? count - done : kDebugChunk;
+        IterArgs a;
+        fill_args(c, seed, first_event + done, n, a);
+        cudaError_t e = inst_debug(c->inst, a, static_cast<int>((n + 127) / 128), 128, c->stream, d_bins, d_x, d_jac, d_f, d_wf, d_pass);
+        auto copy = [&](void* dst, const void* src, size_t bytes) {
+            if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream);
+        };
+        copy(bins ? bins + done * d : nullptr, d_bins, n * d * 4);
+        copy(x ? x + done * d : nullptr, d_x, n * d * 8);
+        copy(jac ? jac + done : nullptr, d_jac, static_cast<size_t>(n) * 8);
+        copy(f ? f + done : nullptr, d_f, static_cast<size_t>(n) * 8);
+        copy(wf ? wf + done : nullptr, d_wf, static_cast<size_t>(n) * 8);
+        copy(pass ? pass + done : nullptr, d_pass, static_cast<size_t>(n) * 4);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);          // the scratch region is reused by the next chunk
+        if (e != cudaSuccess) return fail(VEGAS_ECUDA, "vegas_debug_events: %s", cudaGetErrorString(e));
+    }
     return VEGAS_OK;
 }
 

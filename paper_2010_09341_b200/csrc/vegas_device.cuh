@@ -61,7 +61,8 @@ struct IterArgs {
     unsigned int total_ctas;   // CTAs of all launches of this iteration
     double* slots0;            // base of the slot regions; fin_lanes regions of stride fin_stride, fin_used slots each
     int fin_lanes, fin_stride, fin_used;
-    unsigned long long n_events;
+    unsigned long long n_events;   // events of the whole iteration; 0: this launch is a shard (no S6, NEXT-2)
+    double* partials;          // device: S1.hi, S1.lo, S2.hi, S2.lo, npass, pad[3] -- the 8-double header in front of H
     double* result;            // device: I, sigma, S1, S2, npass, n
     uint32_t* dev_iter;        // graph replays: advanced by S6 (NULL otherwise)
     double* ring;              // graph replays: (I, sigma) log (NULL otherwise)

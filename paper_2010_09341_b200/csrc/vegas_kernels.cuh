@@ -134,7 +134,8 @@ __device__ __forceinline__ void hist_update_batch(double* hlane, int k0, int d, 
 
 __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, int lane_stride, int per_lane,
                                               const unsigned long long* npass, unsigned long long n_events,
-                                              double* result, uint32_t* dev_iter, double* ring, int ring_len);
+                                              double* partials, double* result, uint32_t* dev_iter, double* ring,
+                                              int ring_len);
 
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
@@ -309,22 +310,47 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
     __syncthreads();
     if (sh_last && tid < 32) {
         __threadfence();                                 // see the other CTAs' slots
-        finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.result, a.dev_iter, a.ring,
-                      a.ring_len);
+        finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.partials, a.result,
+                      a.dev_iter, a.ring, a.ring_len);
     }
 }
 
 // ------------------------------------------------------------------------------------------------
-// finalize_warp (S6), run by the first warp of the CTA that finishes last: fixed-order compensated sum of the
-// per-CTA slots, then
+// finalize_warp, run by the first warp of the CTA that finishes last: fixed-order compensated sum of the
+// per-CTA slots into the partials header
+//   partials[0..4] = S1.hi, S1.lo, S2.hi, S2.lo, npass        (H follows the 8-double header in memory)
+// and then, unless this launch is a shard of an iteration that other GPUs share (n_events == 0: the sums are
+// all-reduced first and S6 runs in finalize_kernel), S6:
 //   I = S1/n ; V = (S2/n - I*I)/(n-1) ; sigma = sqrt(max(V, 0)).
 // One warp; lane l folds slots l, l+32, ... (over the per-stream-lane regions) then a shuffle tree: the order
 // depends only on the launch geometry.
 // result[0..5] = I, sigma, S1, S2, npass, n
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long global_timer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+
+__device__ __forceinline__ void estimate_s6(const double* partials, unsigned long long n_events, double* result)
+{
+    const double S1 = __dadd_rn(partials[0], partials[1]), S2 = __dadd_rn(partials[2], partials[3]);
+    const double n = static_cast<double>(n_events);
+    const double I = __ddiv_rn(S1, n);
+    const double V = __ddiv_rn(__dsub_rn(__ddiv_rn(S2, n), __dmul_rn(I, I)), __dsub_rn(n, 1.0));
+    result[0] = I;
+    result[1] = sqrt(V > 0.0 ? V : 0.0);
+    result[2] = S1;
+    result[3] = S2;
+    result[4] = partials[4];
+    result[5] = n;
+}
+
 __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, int lane_stride, int per_lane,
                                               const unsigned long long* npass, unsigned long long n_events,
-                                              double* result, uint32_t* dev_iter, double* ring, int ring_len)
+                                              double* partials, double* result, uint32_t* dev_iter, double* ring,
+                                              int ring_len)
 {
     const int lane = threadIdx.x & 31;
     Comp t1{0.0, 0.0}, t2{0.0, 0.0};
@@ -336,23 +362,33 @@ __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, i
     comp_warp_reduce(t1);
     comp_warp_reduce(t2);
     if (lane == 0) {
-        const double S1 = __dadd_rn(t1.hi, t1.lo), S2 = __dadd_rn(t2.hi, t2.lo);
-        const double n = static_cast<double>(n_events);
-        const double I = __ddiv_rn(S1, n);
-        const double V = __ddiv_rn(__dsub_rn(__ddiv_rn(S2, n), __dmul_rn(I, I)), __dsub_rn(n, 1.0));
-        result[0] = I;
-        result[1] = sqrt(V > 0.0 ? V : 0.0);
-        result[2] = S1;
-        result[3] = S2;
-        result[4] = static_cast<double>(__ldcg(npass));
-        result[5] = n;
+        // renormalise the pairs so that |lo| <= ulp(hi)/2: sums of pairs from several GPUs stay compensated
+        double h1, l1, h2, l2;
+        two_sum(t1.hi, t1.lo, h1, l1);
+        two_sum(t2.hi, t2.lo, h2, l2);
+        partials[0] = h1; partials[1] = l1; partials[2] = h2; partials[3] = l2;
+        partials[4] = static_cast<double>(__ldcg(npass));
+        if (n_events == 0ull) return;                    // shard: S6 after the all-reduce (finalize_kernel)
+        estimate_s6(partials, n_events, result);
         if (ring) {                                      // graph replays: log (I, sigma) and advance the counter
             const uint32_t it = *dev_iter;
-            ring[2 * (it % ring_len) + 0] = I;
-            ring[2 * (it % ring_len) + 1] = result[1];
+            ring[3 * (it % ring_len) + 0] = result[0];
+            ring[3 * (it % ring_len) + 1] = result[1];
+            ring[3 * (it % ring_len) + 2] = __longlong_as_double(static_cast<long long>(global_timer_ns()));   // log_time
             *dev_iter = it + 1u;
         }
     }
+}
+
+// Time stamp (ns, %globaltimer) written at the start of a graph-replayed run: the first iteration's device time is
+// measured from it, every later one from the previous iteration's S6 (PAPER.md:L79 log_time).
+__global__ void stamp_kernel(double* slot) { *slot = __longlong_as_double(static_cast<long long>(global_timer_ns())); }
+
+// S6 from the partials header after the sums of all shards were added (NEXT-2: one all-reduce per iteration of
+// {S1.hi, S1.lo, S2.hi, S2.lo, npass, pad[3], H[d*N]}).  One thread.
+__global__ void finalize_kernel(const double* __restrict__ partials, unsigned long long n_events, double* __restrict__ result)
+{
+    if (threadIdx.x == 0 && blockIdx.x == 0) estimate_s6(partials, n_events, result);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -386,38 +422,48 @@ __global__ void build_table_kernel(double* __restrict__ edges, void* __restrict_
     }
 }
 
-// refine_kernel (S7, steps 1-6 + the monotonicity check of step 7): one CTA per dimension.  Sums and
-// prefix sums are sequential in ascending i (one thread), exactly the order the definition states; the
-// per-bin work (smoothing, damping, edge interpolation) is spread over the threads.
+// refine_dimension (S7, steps 1-6 + the monotonicity check of step 7): one CTA per dimension.
+// The three sums the definition states as sequential (step 1 total, step 3 normalisation, step 5 prefix sums) keep
+// exactly that order -- one thread each, over shared memory, unrolled so that the loads run ahead of the dependent
+// adds (steps 1 and 3 run at the same time in two different warps); everything per-bin (smoothing, damping, edge
+// interpolation) is spread over the threads.  Step 6's search for "the smallest i with c_{i+1} >= t and m_i > 0" is a
+// binary search over the non-decreasing prefix sums: the smallest i with c_{i+1} >= t has c_i < t <= c_{i+1}, hence
+// m_i > 0, so it is the same bin the linear scan of the definition finds (N-1 if there is none).
 //   new_edges[k][*] receives the candidate edges; flags[k] = 0 ok / 1 not strictly increasing.
+__device__ __forceinline__ double serial_sum(const double* v, int n)
+{
+    double acc = 0.0;
+    int i = 0;
+    for (; i + 8 <= n; i += 8) {
+        const double a0 = v[i], a1 = v[i + 1], a2 = v[i + 2], a3 = v[i + 3], a4 = v[i + 4], a5 = v[i + 5], a6 = v[i + 6], a7 = v[i + 7];
+        acc = __dadd_rn(acc, a0); acc = __dadd_rn(acc, a1); acc = __dadd_rn(acc, a2); acc = __dadd_rn(acc, a3);
+        acc = __dadd_rn(acc, a4); acc = __dadd_rn(acc, a5); acc = __dadd_rn(acc, a6); acc = __dadd_rn(acc, a7);
+    }
+    for (; i < n; ++i) acc = __dadd_rn(acc, v[i]);
+    return acc;
+}
+
 __device__ __forceinline__ void refine_dimension(const double* edges, const double* hist, int N, double alpha,
                                                  double* new_edges, int* flags)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* s = reinterpret_cast<double*>(smem_raw);   // [N]   smoothed
+    double* h = reinterpret_cast<double*>(smem_raw);   // [N]   histogram row
+    double* s = h + N;                                  // [N]   smoothed
     double* m = s + N;                                  // [N]   damped weights
     double* cum = m + N;                                // [N+1] prefix sums
-    __shared__ double sh_scalar;
+    double* E = cum + N + 1;                            // [N+1] old edges
+    __shared__ double sh_tot, sh_ssum, sh_delta;
     __shared__ int sh_bad;
 
     const int k = blockIdx.x, tid = threadIdx.x;
-    const double* h = hist + static_cast<size_t>(k) * N;
-    const double* E = edges + static_cast<size_t>(k) * (N + 1);
+    const double* hg = hist + static_cast<size_t>(k) * N;
+    const double* Eg = edges + static_cast<size_t>(k) * (N + 1);
     double* En = new_edges + static_cast<size_t>(k) * (N + 1);
 
-    if (tid == 0) {                                     // step 1
-        double tot = 0.0;
-        for (int i = 0; i < N; ++i) tot = __dadd_rn(tot, h[i]);
-        sh_scalar = tot;
-        sh_bad = 0;
-    }
+    for (int i = tid; i < N; i += blockDim.x) h[i] = hg[i];
+    for (int i = tid; i <= N; i += blockDim.x) E[i] = Eg[i];
+    if (tid == 0) sh_bad = 0;
     __syncthreads();
-    const double tot = sh_scalar;
-    if (!(tot > 0.0) || !isfinite(tot)) {               // nothing to adapt to: dimension unchanged
-        for (int i = tid; i <= N; i += blockDim.x) En[i] = E[i];
-        if (tid == 0) flags[k] = 0;
-        return;
-    }
     for (int i = tid; i < N; i += blockDim.x) {         // step 2
         double v;
         if (i == 0) v = __ddiv_rn(__dadd_rn(h[0], h[1]), 2.0);
@@ -425,14 +471,17 @@ __device__ __forceinline__ void refine_dimension(const double* edges, const doub
         else v = __ddiv_rn(__dadd_rn(__dadd_rn(h[i - 1], h[i]), h[i + 1]), 3.0);
         s[i] = v;
     }
+    if (tid == 0) sh_tot = serial_sum(h, N);            // step 1 (thread 0 smooths its own bins first: h is complete)
     __syncthreads();
-    if (tid == 0) {                                     // step 3
-        double ssum = 0.0;
-        for (int i = 0; i < N; ++i) ssum = __dadd_rn(ssum, s[i]);
-        sh_scalar = ssum;
+    const double tot = sh_tot;
+    if (!(tot > 0.0) || !isfinite(tot)) {               // nothing to adapt to: dimension unchanged
+        for (int i = tid; i <= N; i += blockDim.x) En[i] = E[i];
+        if (tid == 0) flags[k] = 0;
+        return;
     }
+    if (tid == 0) sh_ssum = serial_sum(s, N);           // step 3
     __syncthreads();
-    const double ssum = sh_scalar;
+    const double ssum = sh_ssum;
     for (int i = tid; i < N; i += blockDim.x) {         // step 4
         const double r = __ddiv_rn(s[i], ssum);
         double v;
@@ -445,19 +494,31 @@ __device__ __forceinline__ void refine_dimension(const double* edges, const doub
     if (tid == 0) {                                     // step 5
         double c = 0.0;
         cum[0] = 0.0;
-        for (int i = 0; i < N; ++i) { c = __dadd_rn(c, m[i]); cum[i + 1] = c; }
-        sh_scalar = __ddiv_rn(c, static_cast<double>(N));
+        int i = 0;
+        for (; i + 8 <= N; i += 8) {
+            double a[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) a[j] = m[i + j];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { c = __dadd_rn(c, a[j]); cum[i + j + 1] = c; }
+        }
+        for (; i < N; ++i) { c = __dadd_rn(c, m[i]); cum[i + 1] = c; }
+        sh_delta = __ddiv_rn(c, static_cast<double>(N));
     }
     __syncthreads();
-    const double delta = sh_scalar;
+    const double delta = sh_delta;
     for (int j = tid; j <= N; j += blockDim.x) {        // step 6
         double v;
         if (j == 0) v = 0.0;
         else if (j == N) v = 1.0;
         else {
             const double t = __dmul_rn(static_cast<double>(j), delta);
-            int i = 0;
-            while (i < N - 1 && !(cum[i + 1] >= t && m[i] > 0.0)) ++i;
+            int lo = 0, hi = N - 1;                     // smallest i in [0, N-1] with cum[i+1] >= t, else N-1
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (cum[mid + 1] >= t) hi = mid; else lo = mid + 1;
+            }
+            const int i = lo;
             v = __dadd_rn(E[i], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[i]), m[i]), __dsub_rn(E[i + 1], E[i])));
         }
         En[j] = v;
@@ -471,8 +532,9 @@ __device__ __forceinline__ void refine_dimension(const double* edges, const doub
 
 // refine_kernel (S7): one CTA per dimension computes that dimension's candidate edges (refine_dimension); the
 // CTA that finishes last (ticket counter, __threadfence) does step 7 for all dimensions: if every dimension passed,
-// the candidate edges become the master edges, the table is rebuilt and H is cleared; otherwise nothing changes and
-// status[0] is set to 1 (sticky: the host clears it when it collects the outcome of the refinements enqueued since).
+// the candidate edges become the master edges, the table is rebuilt and H is cleared; otherwise nothing changes (H
+// included, so the caller may refine again, e.g. with another alpha) and status[0] counts the rejection (the host
+// clears it when it collects the outcome of the refinements enqueued since); status[2] = the latest outcome.
 // One launch instead of two: the all-or-nothing commit needs every dimension's flag, i.e. a grid-wide dependency.
 __global__ void refine_kernel(double* edges, const double* hist_in, int N, double alpha, double* new_edges, int* flags,
                               int d, void* table, int precision, double* hist, int* status, unsigned int* ticket)
@@ -491,9 +553,10 @@ __global__ void refine_kernel(double* edges, const double* hist_in, int N, doubl
     for (int j = 0; j < d; ++j) bad |= __ldcg(flags + j);
     if (threadIdx.x == 0) {
         *ticket = 0u;                                    // ready for the next refinement
-        if (bad) status[0] = 1;
+        if (bad) status[0] += 1;                         // refinements rejected since the host last collected
+        status[2] = bad;                                 // outcome of the most recent refinement
     }
-    if (bad) return;
+    if (bad) return;                                     // grid, table and H stay as they were
     const int cells = d * N;
     for (int c = threadIdx.x; c < cells; c += blockDim.x) {
         const int k = c / N, i = c - k * N;

@@ -1,0 +1,45 @@
+"""NEXT-2 ("ensure that all GPUs ... receive a share"): one Vegas iteration
+sharded over the ranks of a torch.distributed process group.
+
+Host logic only -- the partition of the event range and the order of the calls; every step of the arithmetic runs in
+the library's kernels.  Events are counter-indexed (global event index e in [0, n)), so rank g of G runs the events
+[first_g, first_g + count_g) and the ONLY exchange per iteration is one all-reduce (sum) of the unreduced partials
+{S1.hi, S1.lo, S2.hi, S2.lo, npass, 0, 0, 0, H[dim][nbins]} -- 8 + dim*nbins doubles, NCCL over NVLink on GPUs; after
+it every rank holds the same sums, runs S6 (vegas_finalize_enqueue) and the identical refinement, so the grids stay
+bit-identical on all ranks with no further communication.
+
+`ctx` is anything with the binding's three calls (paper_2010_09341_b200.vegas.Vegas, or a stand-in in the CPU tests):
+iterate_shard_enqueue(n_total, first, count, events_per_launch, seed), partials_tensor(), finalize_enqueue(n_total).
+"""
+from __future__ import annotations
+
+
+def shard_range(n_events: int, rank: int, world: int):
+    """(first, count) of rank's share of [0, n_events): equal shares of n // world events, the last rank also takes the
+    remainder.  The shares tile [0, n_events) exactly, in rank order."""
+    if not (0 <= rank < world) or n_events < 0:
+        raise ValueError("rank %d of %d, n_events %d" % (rank, world, n_events))
+    base = n_events // world
+    first = rank * base
+    count = base if rank < world - 1 else n_events - first
+    return first, count
+
+
+def iterate_sharded_enqueue(ctx, n_events: int, events_per_launch: int = 0, seed: int = 0, group=None,
+                            rank: int | None = None, world: int | None = None):
+    """One sharded iteration: this rank's shard, ONE all-reduce of the partials, S6.  Returns the number of kernels this
+    rank launched for its shard.  Without an initialised process group (or world == 1) the shard is the whole range and
+    no collective runs.  Results are read afterwards with ctx.iterate_collect() like after a plain iteration."""
+    import torch.distributed as dist
+    have_pg = dist.is_available() and dist.is_initialized()
+    if world is None:
+        world = dist.get_world_size(group) if have_pg else 1
+    if rank is None:
+        rank = dist.get_rank(group) if have_pg else 0
+    first, count = shard_range(int(n_events), rank, world)
+    epl = int(events_per_launch) if events_per_launch else max(count, 1)
+    launches = ctx.iterate_shard_enqueue(int(n_events), first, count, epl, seed)
+    if world > 1:
+        dist.all_reduce(ctx.partials_tensor(), op=dist.ReduceOp.SUM, group=group)   # the iteration's one exchange
+    ctx.finalize_enqueue(int(n_events))
+    return launches

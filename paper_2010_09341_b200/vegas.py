@@ -41,6 +41,10 @@ SIGNATURES = {
     "vegas_last_npass": (C.c_int, [_vp, _u64p]),
     "vegas_iterate_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, _ip]),
     "vegas_iterate_collect": (C.c_int, [_vp, _dp, _dp, _dp]),
+    "vegas_iterate_shard_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, _ip]),
+    "vegas_partials": (C.c_int, [_vp, C.POINTER(_vp), _szp]),
+    "vegas_finalize_enqueue": (C.c_int, [_vp, C.c_uint64]),
+    "vegas_set_histogram": (C.c_int, [_vp, _dp]),
     "vegas_set_launch_shape": (C.c_int, [_vp, C.c_int, C.c_int]),
     "vegas_set_hist_replicas": (C.c_int, [_vp, C.c_int]),
     "vegas_get_launch_shape": (C.c_int, [_vp, _ip, _ip, _ip, _szp]),
@@ -145,7 +149,10 @@ class Vegas:
         _chk(lib().vegas_refine(self._h, float(alpha)), "vegas_refine")
 
     def run_integration(self, n_iter, n_events, events_per_launch=0, seed=0, alpha=1.5, n_warmup=0):
-        """PAPER.md:L79 run_integration: returns (mean, error, chi2_dof, per-iteration dict)."""
+        """PAPER.md:L79 run_integration: returns (mean, error, chi2_dof, per-iteration dict).  kernel_ms[i] is the
+        device time of iteration i: with CUDA-graph replay (the default) from the end of iteration i-1 (the start of
+        the run for i = 0) to the end of iteration i, refinement i-1 included (device time stamps); with
+        use_cuda_graph(False) the CUDA-event time of iteration i's kernels alone."""
         n_events = int(n_events)
         epl = int(events_per_launch) if events_per_launch else n_events
         tot = n_iter + n_warmup
@@ -193,6 +200,35 @@ class Vegas:
         _chk(lib().vegas_iterate_collect(self._h, C.byref(I), C.byref(s), _d(h) if want_hist else None),
              "vegas_iterate_collect")
         return I.value, s.value, h
+
+    # ---- NEXT-2: one shard of an iteration, the partials region, S6 after the all-reduce --------------
+    def iterate_shard_enqueue(self, n_total, first, count, events_per_launch=0, seed=0):
+        epl = int(events_per_launch) if events_per_launch else max(int(count), 1)
+        nl = C.c_int()
+        _chk(lib().vegas_iterate_shard_enqueue(self._h, int(n_total), int(first), int(count), epl, int(seed),
+                                               C.byref(nl)), "vegas_iterate_shard_enqueue")
+        return nl.value
+
+    def partials(self):
+        """(device pointer, number of doubles) of {S1.hi, S1.lo, S2.hi, S2.lo, npass, 0, 0, 0, H[dim][nbins]}."""
+        ptr, n = _vp(), C.c_size_t()
+        _chk(lib().vegas_partials(self._h, C.byref(ptr), C.byref(n)), "vegas_partials")
+        return int(ptr.value), int(n.value)
+
+    def partials_tensor(self):
+        """The partials region as a float64 torch tensor sharing the workspace's memory (for all_reduce)."""
+        import torch
+        ptr, n = self.partials()
+        off = ptr - self._ws.data_ptr()
+        return self._ws[off:off + 8 * n].view(torch.float64)
+
+    def finalize_enqueue(self, n_total):
+        _chk(lib().vegas_finalize_enqueue(self._h, int(n_total)), "vegas_finalize_enqueue")
+
+    def set_histogram(self, hist):
+        h = np.ascontiguousarray(hist, dtype=np.float64)
+        assert h.shape == (self.dim, self.nbins)
+        _chk(lib().vegas_set_histogram(self._h, _d(h)), "vegas_set_histogram")
 
     # ---- state ---------------------------------------------------------------------------------------
     def get_grid(self):

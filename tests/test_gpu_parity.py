@@ -148,18 +148,31 @@ def test_iteration_launch_shapes(V, O):
         assert_iteration_close(g.iterate(n, 0, 3), ores)
 
 
-def test_batch_size_independence(V):
-    """Reading R16: the event index is global, so events_per_launch changes nothing but summation order."""
+@pytest.mark.parametrize("graph", [True, False])
+def test_batch_size_independence(V, O, graph):
+    """Reading R16: the event index is global, so events_per_launch changes nothing but summation order.  Every batch
+    size is compared with the oracle (200 / 20 / 2 / 1 launches: the 1/4- and 1/2-of-the-SMs geometries, with and without
+    the CUDA-graph replay of many-launch iterations) and with the first run."""
     w = W.cfg2()
-    g = V.from_workload(w)
+    g, o = make_pair(V, O, w)
+    g.use_cuda_graph(graph)
+    n = 2 * 10**6
+    ores = o.iterate(n, 0, threads=THREADS)
     ref = None
     for epl in (10**4, 10**5, 10**6, 2 * 10**6):
         g.reset()
-        I, s, h = g.iterate(2 * 10**6, epl, 0)
+        I, s, h = g.iterate(n, epl, 0)
+        assert_iteration_close((I, s, h), ores)
         if ref is None:
             ref = (I, s, h)
         assert abs(I - ref[0]) <= 1e-13 * abs(ref[0]) and abs(s - ref[1]) <= 1e-13 * abs(ref[1])
         np.testing.assert_allclose(h, ref[2], rtol=1e-12)
+    # a second replay of the cached graph runs the next iteration counter, not the captured one
+    g.reset(); o.reset()
+    for it in range(2):
+        ores = o.iterate(n, 0, threads=THREADS)
+        assert_iteration_close(g.iterate(n, 10**4, 0), ores)
+        assert g.iteration == o.iteration == it + 1
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -346,6 +359,96 @@ def test_full_size_iteration_parity(V, O, name):
         g.refine(w.alpha)
         assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
         g.set_grid(o.get_grid())
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
+def test_full_size_cascade(V, O, name):
+    """BASELINE.json acceptance at the stated sizes: 5 free-running iterations of 1e8 events (the GPU grid is never
+    re-seeded from the oracle), refine after each.  I, sigma rel 1e-12, every H cell rel 1e-10, the pass count exact in
+    every iteration; refined edges within 1e-12 (absolute) of the oracle's after every refinement, the fifth included."""
+    w = small_workloads()[name]
+    assert w.n_events == 10**8
+    g, o = make_pair(V, O, w)
+    for it in range(5):
+        ores = o.iterate(w.n_events, w.seed, threads=THREADS)
+        gres = g.iterate(w.n_events, 0, w.seed)
+        assert_iteration_close(gres, ores)
+        if o.npass is not None:
+            assert g.last_npass() == o.npass
+        o.refine(w.alpha)
+        g.refine(w.alpha)
+        ge, oe = g.get_grid(), o.get_grid()
+        assert np.all(np.diff(ge, axis=1) > 0) and np.all(ge[:, 0] == 0) and np.all(ge[:, -1] == 1)
+        assert np.max(np.abs(ge - oe)) <= 1e-12, (it, np.max(np.abs(ge - oe)))
+    assert g.iteration == o.iteration == 5
+
+
+def test_cfg3_sweep_parity(V, O):
+    """BASELINE.json configs[2]: 1e8 events of the d=8 double Gaussian split into launches of 1e4 ... 1e8 events; every
+    split is compared with ONE oracle iteration (not with another GPU run).  10 000 / 1 000 launches run on 1/8 of the
+    SMs each over 8 internal streams (as a replayed CUDA graph, and for 1e4 / 1e5 also as plain launches), 100 on 1/4,
+    10 on 1/2, 1 on all."""
+    w = W.cfg3()
+    g, o = make_pair(V, O, w)
+    ores = o.iterate(w.n_events, w.seed, threads=THREADS)
+    for epl, graph in [(e, True) for e in w.batch_sizes] + [(10**4, False), (10**5, False)]:
+        g.reset()
+        g.use_cuda_graph(graph)
+        gres = g.iterate(w.n_events, epl, w.seed)
+        assert_iteration_close(gres, ores)
+        S1, S2, _ = g.last_sums()
+        oS1, oS2 = o.last_sums()
+        assert abs(S1 - oS1) <= 1e-12 * abs(oS1) and abs(S2 - oS2) <= 1e-12 * abs(oS2)
+        np.testing.assert_allclose(gres[2].sum(axis=1), S2, rtol=1e-12)
+    # and the cascade of the sweep's smallest batch: 3 free-running iterations at 1e5 events per launch
+    g.reset(); o.reset()
+    g.use_cuda_graph(True)
+    for it in range(3):
+        ores = o.iterate(w.n_events, w.seed, threads=THREADS)
+        assert_iteration_close(g.iterate(w.n_events, 10**5, w.seed), ores)
+        o.refine(w.alpha); g.refine(w.alpha)
+        assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+
+
+def test_two_contexts_of_one_generic_instance_interleaved(V, O):
+    """Two live contexts that share one run-time-shaped kernel instance with different shapes (different nbins, hence
+    different dynamic shared memory) do not disturb each other (the shared-memory limit is a per-function attribute)."""
+    wa = W.Workload("gsa", 3, 400, W.GAUSS_SYM, (0.1, 0.5), W.FP64, 10**5, 1)     # large histogram
+    ga, oa = make_pair(V, O, wa)
+    wb = W.Workload("gsb", 3, 8, W.GAUSS_SYM, (0.1, 0.5), W.FP64, 10**5, 1)       # small one, created afterwards
+    gb, ob = make_pair(V, O, wb)
+    assert ga.launch_shape()["smem_bytes"] > 48 * 1024 > gb.launch_shape()["smem_bytes"]
+    ra, rb = oa.iterate(200_003, 1, threads=THREADS), ob.iterate(200_003, 1, threads=THREADS)
+    for _ in range(2):
+        ga.reset(); gb.reset()
+        assert_iteration_close(ga.iterate(200_003, 0, 1), ra)
+        assert_iteration_close(gb.iterate(200_003, 0, 1), rb)
+
+
+def test_state_after_graph_run_set_grid_and_consumed_histogram(V):
+    """State-machine holes: last_sums() after a graph-replayed run on a fresh context, set_grid dropping the histogram,
+    the histogram being unavailable after a successful refine."""
+    w = W.cfg1()
+    g = V.from_workload(w)
+    m, e, c2, log = g.run_integration(3, 50_000, 0, w.seed, w.alpha)
+    S1, S2, ms = g.last_sums()                          # the run's average step time, not an unrecorded event pair
+    assert ms > 0 and np.all(log["kernel_ms"] > 0)
+    assert abs(ms - log["kernel_ms"].mean()) < 0.5 * ms
+    g.iterate(50_000, 0, w.seed)
+    g.set_grid(g.get_grid())
+    with pytest.raises(V.VegasError) as ei:
+        g.refine(w.alpha)                               # H was sampled through the grid that set_grid replaced
+    assert ei.value.code == V.ESTATE
+    g.iterate(50_000, 0, w.seed)
+    g.refine(w.alpha)
+    with pytest.raises(V.VegasError) as ei:
+        g.iterate_collect(want_hist=True)               # consumed (cleared) by the refinement
+    assert ei.value.code == V.ESTATE
+    I, s, _ = g.iterate_collect(want_hist=False)
+    assert s > 0
+    with pytest.raises(V.VegasError) as ei:
+        g.iterate(10**8, 10, w.seed)                    # 1e7 launches: refused up front
+    assert ei.value.code == V.EINVAL
 
 
 def test_batch_size_study_shape(V):
