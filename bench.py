@@ -8,12 +8,13 @@ BASELINE.json configs[1] (d=8 double Gaussian, 50 bins, 1e8 events per iteration
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg4|cfg5|cfg1] [--epl E]
   python bench.py --impl reference ...      # the CPU oracle, as it stands, on the host cores
 
-Prints ONE JSON line (rank 0).  `value` = events of all ranks / device time (CUDA events, max over ranks);
+Prints ONE JSON line (rank 0).  `value` = events of the whole job / device time (CUDA events, max over ranks);
 `e2e` = the same through vegas_iterate/vegas_refine with host result buffers (D2H of I, sigma, histogram
 inside the timed region; the path has no host inputs: events are generated in registers from
 (seed, iteration, event index)); `roofline` and `cpu_baseline` as described in DESIGN.md "Measurement".
-Multi-GPU: the path does not shard in this build ("replicas only"): --gpus N runs N
-independent replicas, one process per GPU, no data-path collective.
+Multi-GPU (--gpus N under torchrun): the iteration is SHARDED: rank g runs the events
+[g n/N, (g+1) n/N) of the same n-event iteration, ONE all-reduce (NCCL) of the 8 + d*N partial sums per iteration,
+then S6 and the identical refinement on every rank -- total work fixed, "scaling": "strong".
 """
 from __future__ import annotations
 
@@ -39,10 +40,23 @@ UNIT = "events/s"
 ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg2_u32": 154.0, "cfg4": 232.0, "cfg5": (130.0, 14.0)}
 # FP pipe lanes per SM (B200): 64 fp64, 128 fp32.  Peak = SMs * lanes * 2 FLOP * max SM clock.
 FP_LANES = {"f64": 64, "f32": 128}
-# dram__bytes_read.sum + dram__bytes_write.sum of one 1e8-event iterate_kernel launch, from the ncu --set full
-# captures summarised in profiles/r01[c-e]_ncu_full_<cfg>_iterate.md (the algorithmic HBM traffic is ~0: one table
-# read and one d*N flush per CTA)
-NCU_TRAFFIC_BYTES = {"cfg2": 36352, "cfg4": 73216, "cfg5": 44032}   # r01c-r01e captures: 35-44 KB (cfg2, cfg5), 70-73 KB (cfg4)
+# What one launch of the committed iterate kernel executed per event and moved through DRAM, from the round-2 ncu
+# captures (profiles/r02_kernel_counts.md names the commands; written by `python -m paper_2010_09341_b200.ncu_counts`).
+# The algorithmic HBM traffic is ~0: one table read and one d*N flush per CTA.
+KERNEL_COUNTS_CSV = os.path.join(ROOT, "profiles", "r02_kernel_counts.csv")
+
+
+def kernel_counts(workload):
+    """Row of profiles/r02_kernel_counts.csv for this workload (dict of floats), or None."""
+    import csv
+    try:
+        with open(KERNEL_COUNTS_CSV) as fh:
+            for row in csv.DictReader(fh):
+                if row["workload"] == workload:
+                    return {k: (float(v) if k not in ("workload", "kernel") else v) for k, v in row.items()}
+    except OSError:
+        pass
+    return None
 
 
 def parse_args():
@@ -60,6 +74,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=10**8, help="events of the cpu_baseline oracle step")
     ap.add_argument("--ref-sample", type=int, default=10**7, help="events per step of --impl reference")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="gloo lets two ranks share one GPU (a check of the sharded path on a 1-GPU box; not a measurement)")
     return ap.parse_args()
 
 
@@ -189,14 +205,29 @@ def max_over_ranks(values, device="cpu"):
     return [float(v) for v in t.tolist()]
 
 
-def aggregate_value(events_per_rank_step, steps, world, ms):
-    """Whole-job throughput of `world` independent replicas: all ranks' events over the slowest rank's time."""
-    return float(events_per_rank_step) * steps * world / (ms * 1e-3)
+def aggregate_value(events_per_step, steps, ms):
+    """Whole-job throughput of the sharded run: the n events of every step (all ranks' shards together) over the slowest
+    rank's time."""
+    return float(events_per_step) * steps / (ms * 1e-3)
+
+
+def nccl_lines(path, limit=12):
+    """The communicator lines NCCL wrote to its debug file (topology / algorithm evidence for the N > 1 run)."""
+    keep = []
+    try:
+        with open(path) as fh:
+            for ln in fh:
+                if any(k in ln for k in ("comm 0x", "NVLS", "Connected all", "nRanks", "Init COMPLETE", "Channel 00/")):
+                    keep.append(ln.strip()[:200])
+    except OSError:
+        pass
+    return keep[:limit]
 
 
 def run_b200(args):
     import torch
     import torch.distributed as dist
+    from paper_2010_09341_b200 import sharded as S
     from paper_2010_09341_b200 import vegas as V
 
     rank = int(os.environ.get("RANK", "0"))
@@ -204,10 +235,19 @@ def run_b200(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    local = local % torch.cuda.device_count()            # (--dist-backend gloo: several ranks may share one GPU)
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    nccl_log = None
     if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
+        if args.dist_backend == "nccl":
+            nccl_log = "/tmp/vegas_bench_nccl_%d.log" % os.getpid()
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT,GRAPH")
+            os.environ.setdefault("NCCL_DEBUG_FILE", nccl_log)
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group("gloo")
 
     def barrier():
         if world > 1:
@@ -215,7 +255,8 @@ def run_b200(args):
         torch.cuda.synchronize(dev)
 
     w, n = workload(args)
-    epl = args.epl or n
+    first, count = S.shard_range(n, rank, world)         # this rank's share of every iteration (all of it at N = 1)
+    epl = args.epl or max(count, 1)
     g = V.from_workload(w, device="cuda:%d" % local)
     if args.ctas_per_sm or args.threads:
         g.set_launch_shape(args.ctas_per_sm, args.threads)
@@ -228,7 +269,10 @@ def run_b200(args):
              ("imad_wide", V.PIPE_IMAD_WIDE), ("lop3", V.PIPE_LOP3), ("shared_f64_add", V.PIPE_SHARED_F64_ADD))} if rank == 0 else {}
 
     def step_async():
-        nl = g.iterate_enqueue(n, epl, w.seed)
+        if world == 1:
+            nl = g.iterate_enqueue(n, epl, w.seed)
+        else:                               # this rank's shard, ONE all-reduce of the 8 + d*N partials, S6 on every rank
+            nl = S.iterate_sharded_enqueue(g, n, epl, w.seed) + 1
         g.refine_enqueue(w.alpha)           # S7, no host round trip; outcome collected after the timed region
         return nl + 1                       # iterate launches (S6 runs in their last CTA) + the refine kernel
 
@@ -257,35 +301,64 @@ def run_b200(args):
     pass_fraction = g.last_npass() / float(n)
 
     # ---- end-to-end region: the public blocking calls with host result buffers ----
+    def step_blocking():
+        if world == 1:
+            g.iterate(n, epl, w.seed)                   # D2H: I, sigma, histogram
+        else:
+            S.iterate_sharded_enqueue(g, n, epl, w.seed)
+            g.iterate_collect()                         # D2H: I, sigma, histogram
+        g.refine(w.alpha)                               # D2H: status
+
     g.reset()
     for _ in range(args.warmup):
-        g.iterate(n, epl, w.seed)
-        g.refine(w.alpha)
+        step_blocking()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        g.iterate(n, epl, w.seed)           # D2H: I, sigma, histogram
-        g.refine(w.alpha)
+        step_blocking()
     torch.cuda.synchronize(dev)
     e2e_ms = (time.perf_counter() - t0) * 1e3
 
-    dev_ms, e2e_ms, iter_ms = max_over_ranks([dev_ms, e2e_ms, iter_ms], dev)
+    dev_ms, e2e_ms, iter_ms = max_over_ranks([dev_ms, e2e_ms, iter_ms], dev if args.dist_backend == "nccl" else "cpu")
 
     if rank == 0:
-        total_events = float(n) * args.steps * world
-        value = aggregate_value(n, args.steps, world, dev_ms)
+        total_events = float(n) * args.steps              # the whole job: every step is ONE n-event iteration
+        value = aggregate_value(n, args.steps, dev_ms)
         dt = dtype_of(w)
-        kern_s = iter_ms * 1e-3 / args.steps          # average duration of one iteration's kernels
+        kern_s = iter_ms * 1e-3 / args.steps          # average duration of one iteration's kernels (this rank's shard)
         fpe = ALGO_FLOPS[args.workload]
         if isinstance(fpe, tuple):
             fpe = fpe[0] * pass_fraction + fpe[1] * (1.0 - pass_fraction)
-        flops = fpe * n
-        peak = info["sm_count"] * FP_LANES[dt] * 2 * (clocks.get("sm_max_mhz") or info["sm_clock_khz"] / 1e3) * 1e6 / 1e12
+        flops = fpe * count                           # one rank's launch processes its shard
+        clock_hz = (clocks.get("sm_max_mhz") or info["sm_clock_khz"] / 1e3) * 1e6
+        peak = info["sm_count"] * FP_LANES[dt] * 2 * clock_hz / 1e12
         achieved = flops / kern_s / 1e12
-        peak_measured = 2.0 * pipes["dfma" if dt == "f64" else "ffma"] / 1e12
+        fp_rate = pipes["dfma" if dt == "f64" else "ffma"]
+        peak_measured = 2.0 * fp_rate / 1e12
+        # ---- the four co-bounds (SURVEY 8.d "Report all four"): fraction of each SM resource's measured rate that this
+        # kernel's own instruction stream takes at the measured events/s; per-event counts from the ncu capture of the
+        # committed kernel (profiles/r02_kernel_counts.csv), rates from vegas_pipe_rate in this process
+        kc = kernel_counts(args.workload)
+        ev_per_s = count / kern_s
+        bounds, bound_detail = None, None
+        if kc:
+            issue_rate = info["sm_count"] * 4 * 32 * clock_hz          # one warp instruction per SM sub-partition per cycle
+            bounds = {
+                "fp_pipe": ev_per_s * kc["fp64" if dt == "f64" else "fp32"] / fp_rate,
+                "int_wide": ev_per_s * kc["imad_wide"] / pipes["imad_wide"],
+                "shared_atomic": ev_per_s * w.dim / pipes["shared_f64_add"],
+                "issue": ev_per_s * kc["inst"] / issue_rate,
+            }
+            bound_detail = {"per_event": {k: kc[k] for k in ("inst", "fp64", "fp32", "imad_wide", "imad", "lop3", "lds", "atoms")},
+                            "hist_updates_per_event": w.dim,
+                            "source": "profiles/r02_kernel_counts.csv (ncu capture of %s)" % kc["kernel"],
+                            "meaning": "events/s x per-event count / measured rate of that resource (1.0 = saturated); "
+                                       "shared_atomic counts the d histogram updates against the measured LDS+DADD+ATOMS.CAS update rate"}
+        at_full = (n == w.n_events and world == 1 and epl == n)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": dev_ms / args.steps, "higher_is_better": True, "scaling": "strong" if world > 1 else "weak",
+            "vs_baseline": None,
             "dtype": dt, "data": "synthetic", "config": config_of(args, w, n, shape),
             "clocks": clocks,
             "e2e": {"value": total_events / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 0,
@@ -293,16 +366,25 @@ def run_b200(args):
                     "note": "vegas_iterate + vegas_refine with host result buffers, host wall clock"},
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if n == w.n_events and epl == n else None,
-                         "traffic_unit": "bytes per launch (ncu, profiles/r01c_*)", "kernel": "iterate_kernel", "kernel_ms": kern_s * 1e3,
+                         "traffic": kc["dram_bytes"] if (kc and at_full) else None,
+                         "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture in profiles/r02_kernel_counts.csv",
+                         "kernel": "iterate_kernel", "kernel_ms": kern_s * 1e3,
                          "flops_per_event": fpe,
                          "peak_source": "SMs x %d %s lanes x 2 x max SM clock (B200 unit counts; DESIGN.md section 7)" % (FP_LANES[dt], dt),
                          "peak_measured": peak_measured, "frac_of_measured": achieved / peak_measured,
                          "peak_measured_source": "2 x vegas_pipe_rate(%s) in this process before the timed region" % ("DFMA" if dt == "f64" else "FFMA"),
                          "pipe_rates_thread_instr_per_s": pipes,
-                         "note": "issue-slot and IMAD.WIDE co-bounds: DESIGN.md section 7"},
+                         "bounds": bounds, "co_bound": max(bounds, key=bounds.get) if bounds else None,
+                         "bounds_detail": bound_detail},
             "result": {"integral": I, "error": s, "pass_fraction": pass_fraction},
         }
+        if world > 1:
+            out["config"]["parallelism"] = ("events sharded over %d ranks ([g n/N, (g+1) n/N), last rank takes the remainder); one "
+                                            "all-reduce of %d doubles per iteration (%s); identical refine on every rank"
+                                            % (world, 8 + w.dim * w.nbins, args.dist_backend))
+            out["config"]["nccl"] = nccl_lines(nccl_log) if nccl_log else []
+            for ln in out["config"]["nccl"]:
+                print("[nccl] " + ln, file=sys.stderr)
         if not args.no_cpu_baseline and world == 1:
             ns = min(n, args.cpu_sample)
             cdt, cores = oracle_steps(w, ns, 1, 0)

@@ -24,9 +24,10 @@ using namespace vegas;
 constexpr int kMaxTable = 4096;         // doubles of integrand data (tabulated PDF)
 constexpr int kRing = 64;               // (I, sigma) entries logged on the device between two reads of a graph run
 constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
-constexpr int kLanes = 8;               // internal streams the launches of one iteration are dealt to (a8)
-constexpr int kLaneSlots = 2048;        // slots per lane = upper bound on the iterate grid (CTAs)
-constexpr int kMaxSlots = kLanes * kLaneSlots;
+constexpr int kLanes = 32;              // internal streams the launches of one iteration are dealt to (a8): 8 of them, all 32
+                                        // when there are so many launches that each gets 1/8 of the SMs or less
+constexpr int kLaneSlots = 2048;        // upper bound on the iterate grid (CTAs) = slots of a lane's region
+constexpr int kMaxSlots = 8 * kLaneSlots;   // lanes x (largest grid among the launches) never exceeds this
 constexpr size_t kStaticSmemReserve = 1024;   // the opt-in shared-memory limit covers static + dynamic: room for the kernels' few static words
 constexpr int kPartHeader = 8;          // doubles in front of H: S1.hi, S1.lo, S2.hi, S2.lo, npass, pad[3] (vegas_partials)
 constexpr uint32_t kDebugChunk = 4096;  // events per pass of vegas_debug_events through the workspace's scratch region
@@ -170,9 +171,10 @@ constexpr int queue_entry_bytes()
                launch_debug<F, D>, set_smem_attr<F, D, NB, RS, TREP, HB, MAXT, 1>,                       \
                query_occupancy<F, D, NB, RS, TREP, HB, MAXT, 1>, nullptr, nullptr }
 #define VEGAS_GENERIC(ID, F, D, PREC)                                                                    \
-    Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, queue_entry_bytes<F, D>(), launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,          \
-               launch_debug<F, D>, set_smem_attr<F, D, 0, -1, 1, 0, 1024, 1>,                            \
+    Instance { ID, D, 0, PREC, -1, 1, 1024, 2, 512, queue_entry_bytes<F, D>(), launch_iterate<F, D, 0, -1, 1, 0, 1024, 1>,   \
+               launch_debug<F, D>, set_smem_attr<F, D, 0, -1, 1, 0, 1024, 1>,                     \
                query_occupancy<F, D, 0, -1, 1, 0, 1024, 1>, nullptr, nullptr }
+
 
 const Instance kInstances[] = {
     VEGAS_TUNED(VEGAS_GAUSS_SYM, GaussSym, 4, 50, 5, 8, 4, VEGAS_FP64, 1024, 1, 1024),            // configs[0]
@@ -289,6 +291,7 @@ int setup_integrand(vegas_ctx* c, const double* p)
             double C = 1.0;
             for (int k = 0; k < c->dim; ++k) C = C / b;
             c->ic.gC = C;
+            c->ic.ghalfC = 0.5 * C;
             c->ic.ga2 = 1.0 / (alpha * alpha);
             c->ic.gmu0 = p[1];
             c->ic.gmu1 = (c->integrand_id == VEGAS_GAUSS_DOUBLE) ? p[2] : 0.0;
@@ -768,7 +771,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     // several launches they are dealt round-robin to kLanes internal streams forked from the caller's stream:
     // launches that do not fill the GPU overlap, and every launch's prologue/flush overlaps its neighbours'.
     const uint64_t n_launches = (count + epl - 1) / epl;
-    const int lanes = n_launches > 1 ? kLanes : 1;
+    const int lanes = n_launches >= 64 ? kLanes : n_launches > 1 ? 8 : 1;
     // several launches in flight: each takes a fraction of the SMs, so that one launch's prologue / flush overlaps
     // its neighbours' event loops (a CTA of a tuned instance fills an SM's shared memory: full-size grids cannot
     // share an SM).  The fraction grows with the number of launches (measured on cfg3: 2.03 / 2.16 / 3.11 ms per
@@ -810,7 +813,10 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     a.ticket = reinterpret_cast<unsigned int*>(c->ws + c->L.npass) + 4;   // inside the region cleared by the memset
     a.total_ctas = static_cast<unsigned int>(total_ctas);
     a.slots0 = slots0;
-    a.fin_lanes = lanes; a.fin_stride = kLaneSlots; a.fin_used = used_grid;
+    // slot regions: one per stream lane, used_grid slots each (lanes x used_grid <= kMaxSlots: 32 lanes are only used
+    // with grids of at most 1/8 of the SMs x CTAs per SM <= kLaneSlots / 8)
+    if (static_cast<size_t>(lanes) * used_grid > static_cast<size_t>(kMaxSlots)) return fail(VEGAS_EINVAL, "launch geometry needs more slot regions than the workspace holds");
+    a.fin_lanes = lanes; a.fin_stride = used_grid; a.fin_used = used_grid;
     a.n_events = shard ? 0ull : n_total;
     a.result = reinterpret_cast<double*>(c->ws + c->L.result);
     a.dev_iter = (mode == kGraphStep) ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr;
@@ -824,7 +830,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
         a.count = static_cast<uint32_t>(cnt);
         const int grid = launch_grid(cnt);
         const int ln = launches % lanes;
-        a.slots = slots0 + static_cast<size_t>(ln) * kLaneSlots * 4;
+        a.slots = slots0 + static_cast<size_t>(ln) * used_grid * 4;
         CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
         at += cnt;
         ++launches;

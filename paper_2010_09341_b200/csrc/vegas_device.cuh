@@ -30,7 +30,7 @@ constexpr int kMaxDim = 32;
 // ------------------------------------------------------------------------------------------------
 struct IntegrandConsts {
     // I0 / I1 (gauss_sym, gauss_double): C = (alpha sqrt(pi))^-d, a2 = 1/alpha^2, mu[2]
-    double gC, ga2, gmu0, gmu1;
+    double gC, ga2, gmu0, gmu1, ghalfC;
     // I3 (lo_2to2): s, L = log(tau), cos_cut, pdf_a, L^2/s
     double hs, hL, hcut, ha, hLLs;   // hLLs = L^2/s
     // I2 (genz_osc_peak), fp32: phi, c_k, w_k = 1/c_k^2
@@ -114,12 +114,16 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void bin_frac64(uint32_t w_lo, uint32_t w_hi, uint32_t N, int& i, double& frac)
 {
-    const uint64_t p = static_cast<uint64_t>(w_hi) * static_cast<uint64_t>(N << 20) +
-                       static_cast<uint64_t>(w_lo >> 12) * static_cast<uint64_t>(N);
-    const uint32_t phi = static_cast<uint32_t>(p >> 32);
+    // (w_lo>>12)*N < 2^32: a 32-bit multiply, then one wide multiply-add
+    const uint32_t lp = (w_lo >> 12) * N;
+    uint32_t plo, phi;                                   // p = w_hi * (N << 20) + lp: wide multiply, add with carry
+    asm("{\n\t.reg .u64 t;\n\t.reg .u32 tl, th;\n\tmul.wide.u32 t, %2, %3;\n\tmov.b64 {tl, th}, t;\n\t"
+        "add.cc.u32 %0, tl, %4;\n\taddc.u32 %1, th, 0;\n\t}" : "=r"(plo), "=r"(phi) : "r"(w_hi), "r"(N << 20), "r"(lp));
     i = static_cast<int>(phi >> 20);
-    const uint32_t fh = (phi & 0x000FFFFFu) | 0x3FF00000u;
-    frac = __dadd_rn(__hiloint2double(static_cast<int>(fh), static_cast<int>(static_cast<uint32_t>(p))), -1.0);
+    // the bin sits in bits 20.. of phi: OR-ing it into the exponent field of 1.0 (0x3FF: ten low bits set) changes
+    // nothing as long as the bin index has at most ten bits
+    const uint32_t fh = (N <= 1024u) ? (phi | 0x3FF00000u) : ((phi & 0x000FFFFFu) | 0x3FF00000u);
+    frac = __dadd_rn(__hiloint2double(static_cast<int>(fh), static_cast<int>(plo)), -1.0);
 }
 
 // 32-bit-uniform stream mode (VEGAS_FP64_U32): m = w (32 bits), p = m*N, i = p>>32, frac = (p mod 2^32)/2^32.
@@ -136,6 +140,32 @@ __device__ __forceinline__ void bin_frac32(uint32_t w, uint32_t N, int& i, float
     const uint32_t p = (w >> 9) * N;
     i = static_cast<int>(p >> 23);
     frac = __fadd_rn(__uint_as_float((p & 0x007FFFFFu) | 0x3F800000u), -1.0f);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Shared memory by 32-bit shared-window address: one register per address, cell offsets known at compile time
+// fold into the instruction's immediate, and nothing is spent on generic-to-shared conversion in the event loop.
+// The mapping table is read-only while events are processed (plain asm: the compiler may schedule the loads).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return static_cast<uint32_t>(__cvta_generic_to_shared(p)); }
+
+__device__ __forceinline__ void lds_cell(uint32_t addr, double& lo, double& wd)
+{
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(lo), "=d"(wd) : "r"(addr));
+}
+__device__ __forceinline__ void lds_cell(uint32_t addr, float& lo, float& wd)
+{
+    asm("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(lo), "=f"(wd) : "r"(addr));
+}
+__device__ __forceinline__ void ldg_cell(const void* table, int cell, double& lo, double& wd)
+{
+    const double2 t = static_cast<const double2*>(table)[cell];
+    lo = t.x; wd = t.y;
+}
+__device__ __forceinline__ void ldg_cell(const void* table, int cell, float& lo, float& wd)
+{
+    const float2 t = static_cast<const float2*>(table)[cell];
+    lo = t.x; wd = t.y;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -180,7 +210,7 @@ struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
     {
         const double e1 = exp(-__dmul_rn(s1, c.ga2));
         const double e2 = exp(-__dmul_rn(s2, c.ga2));
-        return __dmul_rn(__dmul_rn(0.5, c.gC), __dadd_rn(e1, e2));
+        return __dmul_rn(c.ghalfC, __dadd_rn(e1, e2));        // ghalfC = fl(0.5*C) (exact), set by the host
     }
 };
 
@@ -335,10 +365,12 @@ struct U32 : F {
 // bins[] receives the d bin indices.  Returns wf = (double)J * (double)f.
 // ------------------------------------------------------------------------------------------------
 // event_front: S1 + S2 + the per-coordinate part of S3.  Leaves the integrand's accumulated state in
-// `integrand` and returns J.
-template <class F, int D, int NB, int TSTRIDE, class BinSink>
-__device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint32_t it, uint32_t e_lo, const void* tab_,
-                                                        int toff, BinSink&& sink, F& integrand)
+// `integrand` and returns J.  The table is either the staged copy in shared memory (TCELL > 0: `tab_smem` is the
+// 32-bit shared address of this lane's copy of cell 0 and cells are TCELL bytes apart) or the master table in global
+// memory (TCELL == 0, the parity hook).
+template <class F, int D, int NB, int TCELL, class BinSink>
+__device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint32_t it, uint32_t e_lo, const void* tab_gmem,
+                                                        uint32_t tab_smem, BinSink&& sink, F& integrand)
 {
     using real = typename F::real;
     constexpr bool kF64 = (sizeof(real) == 8);
@@ -347,59 +379,43 @@ __device__ __forceinline__ typename F::real event_front(const IterArgs& a, uint3
     integrand.begin(a.ic);
     real J = real(1);
     uint32_t r[4] = {0u, 0u, 0u, 0u};
-    if constexpr (kF64) {
-        const double2* tab = static_cast<const double2*>(tab_);
-        const double Nd = static_cast<double>(N);
+    const real Nr = static_cast<real>(N);
 #pragma unroll
-        for (int k = 0; k < (D ? D : kMaxDim); ++k) {
-            if (!D && k >= d) break;
-            int i; double frac;
-            if constexpr (F::kU32) {                     // one 32-bit word per coordinate, four per Philox block
-                if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 2), a, r);
-                const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
-                bin_frac64_u32(w, N, i, frac);
-            } else {                                     // 52 bits of two words per coordinate
-                if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 1), a, r);
-                const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
-                bin_frac64(w_lo, w_hi, N, i, frac);
-            }
-            const double2 t = tab[(k * static_cast<int>(N) + i) * TSTRIDE + toff];
-            const double x = __fma_rn(frac, t.y, t.x);
-            const double g = __dmul_rn(Nd, t.y);
-            J = (k == 0) ? g : __dmul_rn(J, g);
-            sink(k, i, x);
-            integrand.coord(k, x, a.ic);
-        }
-    } else {
-        const float2* tab = static_cast<const float2*>(tab_);
-        const float Nf = static_cast<float>(N);
-#pragma unroll
-        for (int k = 0; k < (D ? D : kMaxDim); ++k) {
-            if (!D && k >= d) break;
+    for (int k = 0; k < (D ? D : kMaxDim); ++k) {
+        if (!D && k >= d) break;
+        int i; real frac;
+        if constexpr (kF64 && !F::kU32) {                // 52 bits of two words per coordinate
+            if ((k & 1) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 1), a, r);
+            const uint32_t w_lo = (k & 1) ? r[2] : r[0], w_hi = (k & 1) ? r[3] : r[1];
+            bin_frac64(w_lo, w_hi, N, i, frac);
+        } else {                                         // one 32-bit word per coordinate, four per Philox block
             if ((k & 3) == 0) philox4x32_10(e_lo, a.e_hi, it, static_cast<uint32_t>(k >> 2), a, r);
             const uint32_t w = ((k & 3) == 0) ? r[0] : ((k & 3) == 1) ? r[1] : ((k & 3) == 2) ? r[2] : r[3];
-            int i; float frac;
-            bin_frac32(w, N, i, frac);
-            const float2 t = tab[(k * static_cast<int>(N) + i) * TSTRIDE + toff];
-            const float x = __fmaf_rn(frac, t.y, t.x);
-            const float g = __fmul_rn(Nf, t.y);
-            J = (k == 0) ? g : __fmul_rn(J, g);
-            sink(k, i, x);
-            integrand.coord(k, x, a.ic);
+            if constexpr (kF64) bin_frac64_u32(w, N, i, frac); else bin_frac32(w, N, i, frac);
         }
+        real lo, wd;
+        if constexpr (TCELL > 0)                         // k*N*TCELL is an immediate when D and NB are compile-time
+            lds_cell(tab_smem + static_cast<uint32_t>(k) * N * TCELL + static_cast<uint32_t>(i) * TCELL, lo, wd);
+        else
+            ldg_cell(tab_gmem, k * static_cast<int>(N) + i, lo, wd);
+        real x, g;
+        if constexpr (kF64) { x = __fma_rn(frac, wd, lo); g = __dmul_rn(Nr, wd); J = (k == 0) ? g : __dmul_rn(J, g); }
+        else { x = __fmaf_rn(frac, wd, lo); g = __fmul_rn(Nr, wd); J = (k == 0) ? g : __fmul_rn(J, g); }
+        sink(k, i, x);
+        integrand.coord(k, x, a.ic);
     }
     return J;
 }
 
 // One whole event, S1-S4: returns wf = (double)J * (double)f.
-template <class F, int D, int NB, int TSTRIDE, class BinSink>
-__device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo, const void* tab_, int toff,
+template <class F, int D, class BinSink>
+__device__ __forceinline__ double process_event(const IterArgs& a, uint32_t e_lo, const void* tab_gmem,
                                                 BinSink&& sink, typename F::real& J_out,
                                                 typename F::real& f_out, bool& pass)
 {
     using real = typename F::real;
     F integrand;
-    const real J = event_front<F, D, NB, TSTRIDE>(a, a.iteration, e_lo, tab_, toff, sink, integrand);
+    const real J = event_front<F, D, 0, 0>(a, a.iteration, e_lo, tab_gmem, 0u, sink, integrand);
     pass = integrand.precheck(a.ic);
     const real f = pass ? integrand.end(a.ic, D ? D : a.dim) : real(0);
     J_out = J;

@@ -87,49 +87,91 @@ struct BinPack {   // d bin indices, 16 bits each, kept in registers (all indice
     __device__ __forceinline__ int get(int k) const { return static_cast<int>((w[k >> 1] >> ((k & 1) * 16)) & 0xFFFFu); }
 };
 
-__device__ __forceinline__ unsigned long long lds_u64(const double* p)
+// fp64 histogram cells in shared memory, addressed by 32-bit shared-window address.  On sm_100a an fp64 add on shared
+// memory is a compare-and-swap loop (LDS.64, DADD, ATOMS.CAS.64); written out here so that several chains can be
+// issued together and the lost-race test of a whole batch is one predicate.
+__device__ __forceinline__ unsigned long long hist_load(uint32_t addr)
 {
     unsigned long long v;
-    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(static_cast<uint32_t>(__cvta_generic_to_shared(p))) : "memory");
+    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ unsigned long long hist_cas(uint32_t addr, unsigned long long expect, unsigned long long desired)
+{
+    unsigned long long old;
+    asm volatile("atom.shared.cas.b64 %0, [%1], %2, %3;" : "=l"(old) : "r"(addr), "l"(expect), "l"(desired) : "memory");
+    return old;
+}
+__device__ __forceinline__ unsigned long long add_bits(unsigned long long bits, double q)
+{
+    return static_cast<unsigned long long>(__double_as_longlong(__dadd_rn(__longlong_as_double(static_cast<long long>(bits)), q)));
+}
+// A lost race: one more swap from the value the failed one returned (no reload: the window in which yet another warp
+// can get in between is a DADD long, and on the headline workload this second attempt practically always succeeds);
+// if that is lost too the word is contended (cfg1: all warps of a CTA reach the histogram at the same time) and the
+// update falls back to atomicAdd, which on an fp64 word in shared memory is the loop LDS.64, DADD, ATOMS.CAST.SPIN.64,
+// branch.  (Measured: retrying with plain ATOMS.CAS.64 in a loop costs cfg1 40 % more shared-atomic wavefronts and
+// 5 us per launch; going to atomicAdd straight away costs cfg2 3 %.)
+__device__ __forceinline__ void hist_retry(uint32_t addr, unsigned long long seen, double q)
+{
+    const unsigned long long again = hist_cas(addr, seen, add_bits(seen, q));
+    if (again != seen) atomicAdd(static_cast<double*>(__cvta_shared_to_generic(addr)), q);
+}
+
+// H[k][bin_k] += q for the dims [k0, k0 + HB): all loads, then all adds, then all compare-and-swaps, so the HB
+// dependent chains (LDS -> DADD -> ATOMS.CAS) overlap; the differences (returned ^ expected) are OR-ed into one
+// word (two three-input logic ops per update, opaque to the compiler so that it does not turn them into a
+// predicate per update) and tested once; a lost race (another warp updated the same replica word in between -- rare
+// with lane-indexed replicas) is redone by hist_retry.  `hist_lane` = shared address of this lane's replica of
+// cell 0; cells are HCELL bytes apart (0: run-time, 8 << rs).
+__device__ __forceinline__ uint32_t or_xor(uint32_t acc, uint32_t a, uint32_t b)
+{
+    uint32_t v = acc | (a ^ b);                          // one three-input logic op
+    asm("" : "+r"(v));                                   // opaque: keeps it a data value instead of a predicate chain
     return v;
 }
 
-// H[k][bin_k] += q for the dims [k0, k0 + HB): all loads, then all adds, then all compare-and-swaps, so
-// the HB dependent chains (LDS -> DADD -> ATOMS.CAS) overlap; a lost race (another warp updated the
-// same replica word in between -- rare with lane-indexed replicas) is redone with the spin loop.
-template <int D, int HB>
-__device__ __forceinline__ void hist_update_batch(double* hlane, int k0, int d, int N, int rs, const BinPack<D>& bp,
+template <int D, int NB, int HCELL, int HB>
+__device__ __forceinline__ void hist_update_batch(uint32_t hist_lane, int k0, int d, uint32_t N, int rs, const BinPack<D>& bp,
                                                   double q)
 {
-    double* p[HB];
-    unsigned long long o[HB], n[HB];
+    uint32_t p[HB], off[HB];
+    unsigned long long o[HB], r[HB];
+    uint32_t diff = 0u;
 #pragma unroll
     for (int j = 0; j < HB; ++j) {
         const int k = k0 + j;
         if (k < d) {
-            p[j] = hlane + (static_cast<size_t>(k * N + bp.get(k)) << rs);
-            o[j] = lds_u64(p[j]);
+            if constexpr (HCELL > 0) {
+                p[j] = hist_lane + static_cast<uint32_t>(bp.get(k)) * HCELL;
+                off[j] = static_cast<uint32_t>(k) * N * HCELL;       // an immediate when D and NB are compile-time
+            } else {
+                p[j] = hist_lane + ((static_cast<uint32_t>(k) * N + static_cast<uint32_t>(bp.get(k))) << (3 + rs));
+                off[j] = 0u;
+            }
+            o[j] = hist_load(p[j] + off[j]);
         }
     }
 #pragma unroll
     for (int j = 0; j < HB; ++j)
-        if (k0 + j < d) n[j] = static_cast<unsigned long long>(__double_as_longlong(__dadd_rn(__longlong_as_double(static_cast<long long>(o[j])), q)));
-    bool lost = false;
-    bool lostj[HB];
-#pragma unroll
-    for (int j = 0; j < HB; ++j) {
-        lostj[j] = false;
         if (k0 + j < d) {
-            const unsigned long long r = atomicCAS(reinterpret_cast<unsigned long long*>(p[j]), o[j], n[j]);
-            lostj[j] = (r != o[j]);
-            lost |= lostj[j];
+            r[j] = hist_cas(p[j] + off[j], o[j], add_bits(o[j], q));
+            diff = or_xor(diff, static_cast<uint32_t>(r[j]), static_cast<uint32_t>(o[j]));
+            diff = or_xor(diff, static_cast<uint32_t>(r[j] >> 32), static_cast<uint32_t>(o[j] >> 32));
         }
-    }
-    if (lost) {
+    if (diff != 0u) {
 #pragma unroll
         for (int j = 0; j < HB; ++j)
-            if (lostj[j]) atomicAdd(p[j], q);
+            if (k0 + j < d && r[j] != o[j]) hist_retry(p[j] + off[j], r[j], q);
     }
+}
+
+// one update with the plain spin loop (HB == 0): atomicAdd on an fp64 word in shared memory compiles to the tight loop
+// LDS.64, DADD, ATOMS.CAST.SPIN.64 (swap + success predicate in one instruction), branch -- the form to use when lost
+// races are frequent (few replicas: lanes of one warp that share a replica and a bin collide)
+__device__ __forceinline__ void hist_update_one(double* cell, double q)
+{
+    atomicAdd(cell, q);
 }
 
 __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, int lane_stride, int per_lane,
@@ -165,7 +207,10 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
     }
     __syncthreads();
 
-    double* hlane = sh_hist + (lane & (R - 1));
+    constexpr int kTCell = TREP * static_cast<int>(sizeof(real2));       // bytes between the table copies of two cells
+    constexpr int kHCell = (RS >= 0) ? (8 << (RS >= 0 ? RS : 0)) : 0;    // bytes between two cells' replicas (0: run-time)
+    const uint32_t hist_lane = smem_addr(sh_hist) + static_cast<uint32_t>(lane & (R - 1)) * 8u;
+    const uint32_t tab_lane = smem_addr(sh_tab) + static_cast<uint32_t>(lane & (TREP - 1)) * static_cast<uint32_t>(sizeof(real2));
     Comp s1{0.0, 0.0}, s2{0.0, 0.0};
     unsigned int np = 0;
     const uint32_t stride = gridDim.x * blockDim.x;
@@ -180,13 +225,13 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 #pragma unroll
             for (int k0 = 0; k0 < (D ? D : kMaxDim); k0 += HB) {
                 if (!D && k0 >= d) break;
-                hist_update_batch<D, HB>(hlane, k0, d, N, rs, bp, q);
+                hist_update_batch<D, NB, kHCell, HB>(hist_lane, k0, d, static_cast<uint32_t>(N), rs, bp, q);
             }
         } else {
 #pragma unroll
             for (int k = 0; k < (D ? D : kMaxDim); ++k) {
                 if (!D && k >= d) break;
-                atomicAdd(hlane + (static_cast<size_t>(k * N + bp.get(k)) << rs), q);
+                hist_update_one(sh_hist + (static_cast<size_t>(k * N + bp.get(k)) << rs) + (lane & (R - 1)), q);
             }
         }
     };
@@ -196,8 +241,8 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
             BinPack<D> bp;
             bp.clear();
             F integrand;
-            const real J = event_front<F, D, NB, TREP>(a, it, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
-                                                       [&](int k, int i, real) { bp.set(k, i); }, integrand);
+            const real J = event_front<F, D, NB, kTCell>(a, it, a.e_lo_first + idx, nullptr, tab_lane,
+                                                         [&](int k, int i, real) { bp.set(k, i); }, integrand);
             accumulate(J, integrand.end(a.ic, d), bp);
             np += 1u;
         }
@@ -236,8 +281,8 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
             real J = real(0);
             if (idx < a.count) {
                 bp.clear();
-                J = event_front<F, D, NB, TREP>(a, it, a.e_lo_first + idx, sh_tab, lane & (TREP - 1),
-                                                [&](int k, int i, real) { bp.set(k, i); }, integrand);
+                J = event_front<F, D, NB, kTCell>(a, it, a.e_lo_first + idx, nullptr, tab_lane,
+                                                  [&](int k, int i, real) { bp.set(k, i); }, integrand);
                 pass = integrand.precheck(a.ic);
             }
             const unsigned m = __ballot_sync(0xFFFFFFFFu, pass);
@@ -583,8 +628,8 @@ __global__ void debug_events_kernel(const __grid_constant__ IterArgs a, int32_t*
     const int d = D ? D : a.dim;
     real J, fv;
     bool ps;
-    const double w = process_event<F, D, 0, 1>(
-        a, a.e_lo_first + idx, a.table, 0,
+    const double w = process_event<F, D>(
+        a, a.e_lo_first + idx, a.table,
         [&](int k, int i, real xv) {
             bins[static_cast<size_t>(idx) * d + k] = i;
             x[static_cast<size_t>(idx) * d + k] = static_cast<double>(xv);

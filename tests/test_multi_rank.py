@@ -1,6 +1,6 @@
-"""The N > 1 path on CPU (gloo, world_size 2).  The hot path does not shard in this build ("replicas only",
-DESIGN.md section 10): what N > 1 adds is host logic -- max-over-ranks timing, whole-job aggregation, and the
-rule that only rank 0 prints (and, for --impl reference, only rank 0 works)."""
+"""The N > 1 host logic of bench.py on CPU (gloo, world_size 2): max-over-ranks timing, whole-job aggregation of the
+sharded run, and the rule that only rank 0 prints (and, for --impl reference, only rank 0 works).  The sharded
+iteration itself (partition, one all-reduce, finalize, identical refine) is covered by tests/test_sharding.py."""
 import json
 import os
 import socket
@@ -44,4 +44,4 @@ def test_single_process_max_over_ranks_is_identity():
     sys.path.insert(0, ROOT)
     import bench
     assert bench.max_over_ranks([1.5, 2.5]) == [1.5, 2.5]
-    assert bench.aggregate_value(100, 2, 4, 1000.0) == 800.0
+    assert bench.aggregate_value(100, 2, 1000.0) == 200.0
