@@ -108,10 +108,11 @@ __device__ __forceinline__ unsigned long long add_bits(unsigned long long bits, 
 }
 // A lost race: one more swap from the value the failed one returned (no reload: the window in which yet another warp
 // can get in between is a DADD long, and on the headline workload this second attempt practically always succeeds);
-// if that is lost too the word is contended (cfg1: all warps of a CTA reach the histogram at the same time) and the
-// update falls back to atomicAdd, which on an fp64 word in shared memory is the loop LDS.64, DADD, ATOMS.CAST.SPIN.64,
-// branch.  (Measured: retrying with plain ATOMS.CAS.64 in a loop costs cfg1 40 % more shared-atomic wavefronts and
-// 5 us per launch; going to atomicAdd straight away costs cfg2 3 %.)
+// if that is lost too the word is contended and the update falls back to atomicAdd, which on an fp64 word in shared
+// memory is the loop LDS.64, DADD, ATOMS.CAST.SPIN.64, branch.  Measured: looping on plain
+// ATOMS.CAS.64 with the returned value instead is much worse whenever several lanes or warps really collide -- cfg1
+// (all warps of a CTA reach the histogram together) +40 % shared-atomic wavefronts and +5 us per launch, cfg4 (R = 8:
+// four lanes of a warp share a replica) 4.2 -> 7.7-8.3 ms; going to atomicAdd straight away costs cfg2 3 %.
 __device__ __forceinline__ void hist_retry(uint32_t addr, unsigned long long seen, double q)
 {
     const unsigned long long again = hist_cas(addr, seen, add_bits(seen, q));
