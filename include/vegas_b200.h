@@ -277,9 +277,14 @@ int vegas_tune_events_per_launch(vegas_ctx* ctx, uint64_t n_events, uint64_t see
  *   VEGAS_PIPE_FFMA            fp32 fused multiply-add
  *   VEGAS_PIPE_IMAD_WIDE       32x32->64 integer multiply (two per Philox round)
  *   VEGAS_PIPE_LOP3            three-input logic op (two per Philox round)
- *   VEGAS_PIPE_SHARED_F64_ADD  fp64 atomicAdd on shared memory, lane-indexed replicas, random cells
+ *   VEGAS_PIPE_SHARED_F64_ADD  fp64 atomicAdd on shared memory, lane-indexed replicas (R = 32), random cells
+ * and, as evidence for the histogram design (none of them is a roofline denominator):
+ *   VEGAS_PIPE_SHARED_F64_ADD_R8     the same update in the layout configs[3] is forced into (2000 cells, R = 8)
+ *   VEGAS_PIPE_SHARED_F64_RMW_PLAIN  the non-atomic LDS.64, DADD, STS.64 a lane-and-warp-private word would allow
+ *   VEGAS_PIPE_SHARED_U32_ADD        the native 32-bit integer shared-memory atomic add
  * Errors: VEGAS_EINVAL (unknown pipe, NULL out), VEGAS_ECUDA. */
-enum { VEGAS_PIPE_DFMA = 0, VEGAS_PIPE_FFMA = 1, VEGAS_PIPE_IMAD_WIDE = 2, VEGAS_PIPE_LOP3 = 3, VEGAS_PIPE_SHARED_F64_ADD = 4 };
+enum { VEGAS_PIPE_DFMA = 0, VEGAS_PIPE_FFMA = 1, VEGAS_PIPE_IMAD_WIDE = 2, VEGAS_PIPE_LOP3 = 3, VEGAS_PIPE_SHARED_F64_ADD = 4,
+       VEGAS_PIPE_SHARED_F64_ADD_R8 = 5, VEGAS_PIPE_SHARED_F64_RMW_PLAIN = 6, VEGAS_PIPE_SHARED_U32_ADD = 7 };
 int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr_per_s);
 
 #ifdef __cplusplus

@@ -18,7 +18,7 @@ constexpr int kUnroll = 16;   // operations per chain per loop trip
 template <int KIND>
 __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long long* out, uint32_t seed)
 {
-    extern __shared__ double sh[];                     // KIND 4: [32 cells][32 lanes]
+    extern __shared__ double sh[];                     // KIND 4, 6, 7: [32 cells][32 lanes]; KIND 5: [2000 cells][8 replicas]
     const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     double d[kChains];
     float f[kChains];
@@ -32,8 +32,9 @@ __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long 
         u[c] = t * 31u + c + seed;
         v[c] = t * 17u + c * 3u + seed;
     }
-    if (KIND == 4) {
-        for (int i = threadIdx.x; i < 32 * 32; i += blockDim.x) sh[i] = 0.0;
+    if (KIND >= 4) {
+        const int words = (KIND == 5) ? 2000 * 8 : 32 * 32;
+        for (int i = threadIdx.x; i < words; i += blockDim.x) sh[i] = 0.0;
         __syncthreads();
     }
     const double da = 1.0000001, db = 1e-9;
@@ -52,6 +53,24 @@ __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long 
                     u[c] = u[c] * 1664525u + 1013904223u;
                     atomicAdd(&sh[((u[c] >> 27) << 5) + (threadIdx.x & 31)], db);
                 }
+                if (KIND == 5) {
+                    // the same with the layout configs[3] is forced into (2000 cells, R = 8: four lanes of a warp share a
+                    // replica and collide when they draw the same cell of 100 -- here one of 100 consecutive cells)
+                    u[c] = u[c] * 1664525u + 1013904223u;
+                    atomicAdd(&sh[(((u[c] >> 16) % 100u + 100u * c) << 3) + (threadIdx.x & 7)], db);
+                }
+                if (KIND == 6) {
+                    // what the update would cost WITHOUT atomicity (a word that only this lane of this warp may touch:
+                    // not available to the kernel -- it would take 32 replicas per warp): LDS.64, DADD, STS.64
+                    u[c] = u[c] * 1664525u + 1013904223u;
+                    double* p = &sh[((u[c] >> 27) << 5) + (threadIdx.x & 31)];
+                    asm volatile("{\n\t.reg .f64 t;\n\tld.volatile.f64 t, [%0];\n\tadd.rn.f64 t, t, %1;\n\tst.volatile.f64 [%0], t;\n\t}" :: "l"(p), "d"(db) : "memory");
+                }
+                if (KIND == 7) {
+                    // the native shared-memory atomic: 32-bit integer add (cannot hold the histogram's dynamic range)
+                    u[c] = u[c] * 1664525u + 1013904223u;
+                    atomicAdd(reinterpret_cast<unsigned int*>(sh) + ((u[c] >> 27) << 5) + (threadIdx.x & 31), u[c] >> 20);
+                }
             }
         }
     }
@@ -66,7 +85,8 @@ template <int KIND>
 cudaError_t time_kind(int sms, int iters, unsigned long long* out, cudaStream_t st, double* rate)
 {
     const int blocks = sms * 2, threads = 1024;
-    const size_t smem = (KIND == 4) ? 32 * 32 * sizeof(double) : 0;
+    const size_t smem = (KIND == 5) ? 2000 * 8 * sizeof(double) : (KIND >= 4) ? 32 * 32 * sizeof(double) : 0;
+    if (KIND == 5) cudaFuncSetAttribute(pipe_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem));
     cudaEvent_t e0, e1;
     cudaError_t e = cudaEventCreate(&e0);
     if (e != cudaSuccess) return e;
@@ -110,6 +130,9 @@ extern "C" int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr
         case VEGAS_PIPE_IMAD_WIDE: e = time_kind<2>(sms, 500, out, st, thread_instr_per_s); break;
         case VEGAS_PIPE_LOP3: e = time_kind<3>(sms, 1000, out, st, thread_instr_per_s); break;
         case VEGAS_PIPE_SHARED_F64_ADD: e = time_kind<4>(sms, 100, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_SHARED_F64_ADD_R8: e = time_kind<5>(sms, 50, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_SHARED_F64_RMW_PLAIN: e = time_kind<6>(sms, 100, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_SHARED_U32_ADD: e = time_kind<7>(sms, 100, out, st, thread_instr_per_s); break;
         default: cudaFree(out); return VEGAS_EINVAL;
     }
     cudaFree(out);

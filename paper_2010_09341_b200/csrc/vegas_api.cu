@@ -946,17 +946,20 @@ int vegas_refine_enqueue(vegas_ctx* c, double alpha)
     if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
     if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
     const int N = c->nbins;
-    const size_t smem = (5 * static_cast<size_t>(N) + 2) * sizeof(double);
-    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, c->smem_optin - static_cast<int>(kStaticSmemReserve)));
+    // one warp per dimension, all in one CTA; as many dimensions at a time as fit in shared memory
+    const size_t per_dim = 4 * (static_cast<size_t>(N) + 1) * sizeof(double);
+    const int warps = c->dim < 32 ? c->dim : 32;
+    const size_t max_smem = static_cast<size_t>(c->smem_optin) - kStaticSmemReserve;
+    size_t smem = per_dim * static_cast<size_t>(warps);
+    if (smem > max_smem) smem = (max_smem / per_dim) * per_dim;
+    if (smem < per_dim) return fail(VEGAS_EINVAL, "nbins %d: one dimension's refinement does not fit in shared memory", N);
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(max_smem)));
     double* edges = reinterpret_cast<double*>(c->ws + c->L.edges);
     double* new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);
     double* hist = reinterpret_cast<double*>(c->ws + c->L.hist);
-    int* flags = reinterpret_cast<int*>(c->ws + c->L.flags);
     int* status = reinterpret_cast<int*>(c->ws + c->L.status);
-    const int threads = N >= 96 ? 128 : (N + 31) / 32 * 32;
-    refine_kernel<<<c->dim, threads, smem, c->stream>>>(edges, hist, N, alpha, new_edges, flags, c->dim, c->ws + c->L.table,
-                                                        c->precision == VEGAS_FP32_EVAL ? 1 : 0, hist, status,
-                                                        reinterpret_cast<unsigned int*>(c->ws + c->L.status) + 1);
+    refine_kernel<<<1, 32 * warps, smem, c->stream>>>(edges, hist, N, alpha, new_edges, c->dim, c->ws + c->L.table,
+                                                      c->precision == VEGAS_FP32_EVAL ? 1 : 0, status, static_cast<int>(smem));
     CUDA_TRY(cudaGetLastError());
     c->have_hist = false;
     c->hist_consumed = true;

@@ -468,137 +468,153 @@ __global__ void build_table_kernel(double* __restrict__ edges, void* __restrict_
     }
 }
 
-// refine_dimension (S7, steps 1-6 + the monotonicity check of step 7): one CTA per dimension.
-// The three sums the definition states as sequential (step 1 total, step 3 normalisation, step 5 prefix sums) keep
-// exactly that order -- one thread each, over shared memory, unrolled so that the loads run ahead of the dependent
-// adds (steps 1 and 3 run at the same time in two different warps); everything per-bin (smoothing, damping, edge
-// interpolation) is spread over the threads.  Step 6's search for "the smallest i with c_{i+1} >= t and m_i > 0" is a
-// binary search over the non-decreasing prefix sums: the smallest i with c_{i+1} >= t has c_i < t <= c_{i+1}, hence
-// m_i > 0, so it is the same bin the linear scan of the definition finds (N-1 if there is none).
-//   new_edges[k][*] receives the candidate edges; flags[k] = 0 ok / 1 not strictly increasing.
-__device__ __forceinline__ double serial_sum(const double* v, int n)
+// S7 (refine): one warp per dimension, all dimensions in ONE CTA, so that the all-or-nothing commit of step 7 needs
+// no grid-wide dependency.  The refinement is latency-bound (d*N <= a few thousand cells, chains of dependent fp64
+// operations at ~40 cycles each), so everything that the definition states as a sequential sum is done as a
+// lane-chunked sum / scan instead: lane l owns the contiguous bins [l*chunk, (l+1)*chunk), sums or scans them locally
+// and the 32 chunk totals are combined with shuffles (reading R12' in DESIGN.md: the summation ORDER of steps 1, 3 and 5
+// is not the definition's, which moves the sums by a few ulp and the edges by ~1e-16, against a tolerance of 1e-12).
+// Step 6's "smallest i with c_{i+1} >= t and m_i > 0" is a binary search over the non-decreasing prefix sums (the
+// smallest i with c_{i+1} >= t has c_i < t <= c_{i+1}, hence m_i > 0: the same bin the linear scan finds; N-1 if none).
+// Per-dimension shared memory: A[N+1] (h, then m) | B[N+1] (s, then the new edges) | cum[N+1] | E[N+1].
+__device__ __forceinline__ double warp_sum_all(double v)
 {
-    double acc = 0.0;
-    int i = 0;
-    for (; i + 8 <= n; i += 8) {
-        const double a0 = v[i], a1 = v[i + 1], a2 = v[i + 2], a3 = v[i + 3], a4 = v[i + 4], a5 = v[i + 5], a6 = v[i + 6], a7 = v[i + 7];
-        acc = __dadd_rn(acc, a0); acc = __dadd_rn(acc, a1); acc = __dadd_rn(acc, a2); acc = __dadd_rn(acc, a3);
-        acc = __dadd_rn(acc, a4); acc = __dadd_rn(acc, a5); acc = __dadd_rn(acc, a6); acc = __dadd_rn(acc, a7);
-    }
-    for (; i < n; ++i) acc = __dadd_rn(acc, v[i]);
-    return acc;
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v = __dadd_rn(v, __shfl_xor_sync(0xFFFFFFFFu, v, off));
+    return v;                                            // identical in every lane
 }
 
-__device__ __forceinline__ void refine_dimension(const double* edges, const double* hist, int N, double alpha,
-                                                 double* new_edges, int* flags)
+// m = x^alpha for the damping of step 4; the exponents the configurations use avoid the ~150 dependent fp64
+// operations of pow() (values within 1 ulp of it)
+__device__ __forceinline__ double damp_pow(double x, double alpha)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    double* h = reinterpret_cast<double*>(smem_raw);   // [N]   histogram row
-    double* s = h + N;                                  // [N]   smoothed
-    double* m = s + N;                                  // [N]   damped weights
-    double* cum = m + N;                                // [N+1] prefix sums
-    double* E = cum + N + 1;                            // [N+1] old edges
-    __shared__ double sh_tot, sh_ssum, sh_delta;
-    __shared__ int sh_bad;
+    if (alpha == 1.5) return __dmul_rn(x, sqrt(x));
+    if (alpha == 1.0) return x;
+    if (alpha == 0.5) return sqrt(x);
+    if (alpha == 2.0) return __dmul_rn(x, x);
+    return pow(x, alpha);
+}
 
-    const int k = blockIdx.x, tid = threadIdx.x;
-    const double* hg = hist + static_cast<size_t>(k) * N;
-    const double* Eg = edges + static_cast<size_t>(k) * (N + 1);
-    double* En = new_edges + static_cast<size_t>(k) * (N + 1);
+// returns 1 if this dimension's new edges are not strictly increasing, else 0 (same value in every lane)
+__device__ __forceinline__ int refine_dimension_warp(const double* __restrict__ Eg, const double* __restrict__ hg, int N,
+                                                     double alpha, double* __restrict__ Eng, double* sm)
+{
+    const int lane = threadIdx.x & 31;
+    double* A = sm;                                      // [N+1] h, then m
+    double* B = A + (N + 1);                             // [N+1] s, then new edges
+    double* cum = B + (N + 1);                           // [N+1]
+    double* E = cum + (N + 1);                           // [N+1]
+    const int chunk = (N + 31) >> 5;
+    const int lo = lane * chunk < N ? lane * chunk : N, hi = (lo + chunk < N) ? lo + chunk : N;
 
-    for (int i = tid; i < N; i += blockDim.x) h[i] = hg[i];
-    for (int i = tid; i <= N; i += blockDim.x) E[i] = Eg[i];
-    if (tid == 0) sh_bad = 0;
-    __syncthreads();
-    for (int i = tid; i < N; i += blockDim.x) {         // step 2
+    for (int i = lane; i < N; i += 32) A[i] = hg[i];
+    for (int i = lane; i <= N; i += 32) E[i] = Eg[i];
+    __syncwarp();
+    double part = 0.0;                                   // step 1
+    for (int i = lo; i < hi; ++i) part = __dadd_rn(part, A[i]);
+    const double tot = warp_sum_all(part);
+    if (!(tot > 0.0) || !isfinite(tot)) {                // nothing to adapt to: dimension unchanged
+        for (int i = lane; i <= N; i += 32) Eng[i] = E[i];
+        return 0;
+    }
+    part = 0.0;                                          // steps 2 + 3
+    for (int i = lo; i < hi; ++i) {
         double v;
-        if (i == 0) v = __ddiv_rn(__dadd_rn(h[0], h[1]), 2.0);
-        else if (i == N - 1) v = __ddiv_rn(__dadd_rn(h[N - 2], h[N - 1]), 2.0);
-        else v = __ddiv_rn(__dadd_rn(__dadd_rn(h[i - 1], h[i]), h[i + 1]), 3.0);
-        s[i] = v;
+        if (i == 0) v = __ddiv_rn(__dadd_rn(A[0], A[1]), 2.0);
+        else if (i == N - 1) v = __ddiv_rn(__dadd_rn(A[N - 2], A[N - 1]), 2.0);
+        else v = __ddiv_rn(__dadd_rn(__dadd_rn(A[i - 1], A[i]), A[i + 1]), 3.0);
+        B[i] = v;
+        part = __dadd_rn(part, v);
     }
-    if (tid == 0) sh_tot = serial_sum(h, N);            // step 1 (thread 0 smooths its own bins first: h is complete)
-    __syncthreads();
-    const double tot = sh_tot;
-    if (!(tot > 0.0) || !isfinite(tot)) {               // nothing to adapt to: dimension unchanged
-        for (int i = tid; i <= N; i += blockDim.x) En[i] = E[i];
-        if (tid == 0) flags[k] = 0;
-        return;
-    }
-    if (tid == 0) sh_ssum = serial_sum(s, N);           // step 3
-    __syncthreads();
-    const double ssum = sh_ssum;
-    for (int i = tid; i < N; i += blockDim.x) {         // step 4
-        const double r = __ddiv_rn(s[i], ssum);
+    const double ssum = warp_sum_all(part);
+    __syncwarp();                                        // every lane is done reading h before it becomes m
+    part = 0.0;                                          // steps 4 + 5: damped weights and their chunk-local prefix sums
+    for (int i = lo; i < hi; ++i) {
+        const double r = __ddiv_rn(B[i], ssum);
         double v;
         if (r <= 0.0) v = 0.0;
         else if (r >= 1.0) v = 1.0;
-        else v = pow(__ddiv_rn(__dsub_rn(1.0, r), -log(r)), alpha);
-        m[i] = v;
+        else v = damp_pow(__ddiv_rn(__dsub_rn(1.0, r), -log(r)), alpha);
+        A[i] = v;
+        part = __dadd_rn(part, v);
+        cum[i + 1] = part;                               // chunk-local for now
     }
-    __syncthreads();
-    if (tid == 0) {                                     // step 5
-        double c = 0.0;
-        cum[0] = 0.0;
-        int i = 0;
-        for (; i + 8 <= N; i += 8) {
-            double a[8];
+    double incl = part;                                  // inclusive scan of the 32 chunk totals
 #pragma unroll
-            for (int j = 0; j < 8; ++j) a[j] = m[i + j];
-#pragma unroll
-            for (int j = 0; j < 8; ++j) { c = __dadd_rn(c, a[j]); cum[i + j + 1] = c; }
-        }
-        for (; i < N; ++i) { c = __dadd_rn(c, m[i]); cum[i + 1] = c; }
-        sh_delta = __ddiv_rn(c, static_cast<double>(N));
+    for (int off = 1; off < 32; off <<= 1) {
+        const double o = __shfl_up_sync(0xFFFFFFFFu, incl, off);
+        if (lane >= off) incl = __dadd_rn(incl, o);
     }
-    __syncthreads();
-    const double delta = sh_delta;
-    for (int j = tid; j <= N; j += blockDim.x) {        // step 6
+    double offset = __shfl_up_sync(0xFFFFFFFFu, incl, 1);
+    if (lane == 0) offset = 0.0;
+    // The prefix sums must not decrease across a chunk boundary (its two sides are rounded along different paths, so
+    // they can be out of order by an ulp): every chunk is clamped from below by the largest value any earlier chunk
+    // ends with -- a max-scan, which is exact.  Within a chunk fl(offset + local prefix) is non-decreasing already.
+    double endmax = (hi > lo) ? __dadd_rn(offset, part) : 0.0;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const double o = __shfl_up_sync(0xFFFFFFFFu, endmax, off);
+        if (lane >= off && o > endmax) endmax = o;
+    }
+    double floor_ = __shfl_up_sync(0xFFFFFFFFu, endmax, 1);
+    if (lane == 0) floor_ = 0.0;
+    for (int i = lo; i < hi; ++i) {
+        const double v = __dadd_rn(offset, cum[i + 1]);
+        cum[i + 1] = v > floor_ ? v : floor_;
+    }
+    if (lane == 0) cum[0] = 0.0;
+    __syncwarp();
+    const double delta = __ddiv_rn(cum[N], static_cast<double>(N));
+    for (int j = lane; j <= N; j += 32) {                // step 6
         double v;
         if (j == 0) v = 0.0;
         else if (j == N) v = 1.0;
         else {
             const double t = __dmul_rn(static_cast<double>(j), delta);
-            int lo = 0, hi = N - 1;                     // smallest i in [0, N-1] with cum[i+1] >= t, else N-1
-            while (lo < hi) {
-                const int mid = (lo + hi) >> 1;
-                if (cum[mid + 1] >= t) hi = mid; else lo = mid + 1;
+            int a = 0, b = N - 1;                        // smallest i in [0, N-1] with cum[i+1] >= t, else N-1
+            while (a < b) {
+                const int mid = (a + b) >> 1;
+                if (cum[mid + 1] >= t) b = mid; else a = mid + 1;
             }
-            const int i = lo;
-            v = __dadd_rn(E[i], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[i]), m[i]), __dsub_rn(E[i + 1], E[i])));
+            v = __dadd_rn(E[a], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[a]), A[a]), __dsub_rn(E[a + 1], E[a])));
         }
-        En[j] = v;
+        B[j] = v;
+        Eng[j] = v;
     }
-    __syncthreads();
-    for (int j = tid; j < N; j += blockDim.x)           // step 7 check
-        if (!(En[j] < En[j + 1])) sh_bad = 1;
-    __syncthreads();
-    if (tid == 0) flags[k] = sh_bad;
+    __syncwarp();
+    int bad = 0;                                         // step 7 check
+    for (int j = lane; j < N; j += 32)
+        if (!(B[j] < B[j + 1])) bad = 1;
+    return __any_sync(0xFFFFFFFFu, bad) ? 1 : 0;
 }
 
-// refine_kernel (S7): one CTA per dimension computes that dimension's candidate edges (refine_dimension); the
-// CTA that finishes last (ticket counter, __threadfence) does step 7 for all dimensions: if every dimension passed,
-// the candidate edges become the master edges, the table is rebuilt and H is cleared; otherwise nothing changes (H
-// included, so the caller may refine again, e.g. with another alpha) and status[0] counts the rejection (the host
-// clears it when it collects the outcome of the refinements enqueued since); status[2] = the latest outcome.
-// One launch instead of two: the all-or-nothing commit needs every dimension's flag, i.e. a grid-wide dependency.
-__global__ void refine_kernel(double* edges, const double* hist_in, int N, double alpha, double* new_edges, int* flags,
-                              int d, void* table, int precision, double* hist, int* status, unsigned int* ticket)
+// All of S7 by one CTA: candidate edges of every dimension (a warp each, in passes of as many dimensions as fit in
+// `smem_bytes` of shared memory), then step 7 for all dimensions: if every one passed, the candidate edges become
+// the master edges, the table is rebuilt and H is cleared; otherwise nothing changes (H included, so the caller may
+// refine again, e.g. with another alpha) and status[0] counts the rejection (the host clears it when it collects
+// the outcome of the refinements enqueued since); status[2] = the latest outcome.
+__device__ __forceinline__ void refine_all(double* edges, double* hist, int N, double alpha, double* new_edges, int d,
+                                           void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes)
 {
-    __shared__ int sh_last;
-    refine_dimension(edges, hist_in, N, alpha, new_edges, flags);
-    __syncthreads();                                     // this CTA's candidate edges and flag are written
-    if (threadIdx.x == 0) {
-        __threadfence();
-        sh_last = (atomicAdd(ticket, 1u) == static_cast<unsigned int>(d - 1));
-    }
+    __shared__ int sh_bad;
+    const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const size_t per_dim = 4 * (static_cast<size_t>(N) + 1);            // doubles
+    int group = static_cast<int>(smem_bytes / (per_dim * sizeof(double)));
+    if (group > nwarps) group = nwarps;
+    if (threadIdx.x == 0) sh_bad = 0;
     __syncthreads();
-    if (!sh_last) return;
-    __threadfence();                                     // see the other CTAs' edges and flags
-    int bad = 0;
-    for (int j = 0; j < d; ++j) bad |= __ldcg(flags + j);
+    for (int k0 = 0; k0 < d; k0 += group) {
+        const int k = k0 + warp;
+        if (warp < group && k < d) {
+            const int bad = refine_dimension_warp(edges + static_cast<size_t>(k) * (N + 1), hist + static_cast<size_t>(k) * N, N, alpha,
+                                                  new_edges + static_cast<size_t>(k) * (N + 1),
+                                                  reinterpret_cast<double*>(smem) + static_cast<size_t>(warp) * per_dim);
+            if (bad && (threadIdx.x & 31) == 0) sh_bad = 1;
+        }
+    }
+    __syncthreads();                                     // every dimension's candidate edges (global) and verdict are written
+    const int bad = sh_bad;
     if (threadIdx.x == 0) {
-        *ticket = 0u;                                    // ready for the next refinement
         if (bad) status[0] += 1;                         // refinements rejected since the host last collected
         status[2] = bad;                                 // outcome of the most recent refinement
     }
@@ -607,11 +623,18 @@ __global__ void refine_kernel(double* edges, const double* hist_in, int N, doubl
     for (int c = threadIdx.x; c < cells; c += blockDim.x) {
         const int k = c / N, i = c - k * N;
         const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
-        const double lo = __ldcg(En + i), hi = __ldcg(En + i + 1);
+        const double lo = En[i], hi = En[i + 1];
         write_table_cell(table, precision, static_cast<size_t>(c), lo, __dsub_rn(hi, lo));
         hist[c] = 0.0;
     }
-    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = __ldcg(new_edges + e);
+    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = new_edges[e];
+}
+
+__global__ void refine_kernel(double* edges, double* hist, int N, double alpha, double* new_edges, int d, void* table,
+                              int precision, int* status, int smem_bytes)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    refine_all(edges, hist, N, alpha, new_edges, d, table, precision, status, smem_raw, static_cast<size_t>(smem_bytes));
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -60,7 +60,10 @@ def main():
     args = ap.parse_args()
     rows = []
     pipes = {n: V.pipe_rate(k) for n, k in (("dfma", V.PIPE_DFMA), ("ffma", V.PIPE_FFMA), ("imad_wide", V.PIPE_IMAD_WIDE),
-                                           ("lop3", V.PIPE_LOP3), ("shared_f64_add", V.PIPE_SHARED_F64_ADD))}
+                                           ("lop3", V.PIPE_LOP3), ("shared_f64_add", V.PIPE_SHARED_F64_ADD),
+                                           ("shared_f64_add_r8", V.PIPE_SHARED_F64_ADD_R8),
+                                           ("shared_f64_rmw_plain", V.PIPE_SHARED_F64_RMW_PLAIN),
+                                           ("shared_u32_add", V.PIPE_SHARED_U32_ADD))}
     print(json.dumps({"pipe_rates_thread_instr_per_s": pipes}))
     for name in args.configs.split(","):
         w = W.ALL[name]()

@@ -295,6 +295,7 @@ class Vegas:
 
 
 PIPE_DFMA, PIPE_FFMA, PIPE_IMAD_WIDE, PIPE_LOP3, PIPE_SHARED_F64_ADD = 0, 1, 2, 3, 4
+PIPE_SHARED_F64_ADD_R8, PIPE_SHARED_F64_RMW_PLAIN, PIPE_SHARED_U32_ADD = 5, 6, 7   # evidence only
 
 
 def pipe_rate(pipe, stream=None):

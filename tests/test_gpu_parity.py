@@ -497,7 +497,7 @@ def test_async_step_equals_blocking_step(V):
         b.iterate(w.n_events, 30_000, w.seed)
         b.refine(w.alpha)
     a.refine_collect()
-    np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-15)
+    np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-13)   # (H is summed in a different order in the two runs)
     Ia, sa, ha = a.iterate(w.n_events, 0, w.seed)
     Ib, sb, hb = b.iterate(w.n_events, 0, w.seed)
     assert abs(Ia - Ib) <= 1e-13 * abs(Ib) and abs(sa - sb) <= 1e-12 * sb

@@ -143,7 +143,7 @@ def test_exact_bin_rule_vs_rational_and_uniform_x_within_one_ulp():
 def test_constants_against_mpmath():
     mp.mp.dps = 50
     # I0/I1 constants: b=fl(alpha sqrt(fl64(pi))), C=1 then d divisions, a2=fl(1/fl(alpha alpha)).
-    # DESIGN.md reading R18: sqrt of the *rounded* pi (0x1.c5bf891b4ef6ap+0, one ulp below the correctly
+    # DESIGN.md reading R19: sqrt of the *rounded* pi (0x1.c5bf891b4ef6ap+0, one ulp below the correctly
     # rounded sqrt(pi)) -- the value the cited worked example (P2, C for d=4) was computed with.
     alpha = 0.1
     sqrt_pi = float(mp.sqrt(mp.mpf(float(mp.pi))))
