@@ -2,7 +2,7 @@
 """bench.py -- events/s per Vegas iteration (BASELINE.json metric) on the headline workload.
 
 A step = one pass of the whole hot path: one Vegas iteration over n_events (S1-S6: Philox draw, grid map,
-integrand, compensated sums, histograms, finalize) followed by the grid refinement (S7), on
+integrand, compensated sums, histograms, finalize) followed by the grid refinement (S7) -- vegas_step_enqueue, on
 BASELINE.json configs[1] (d=8 double Gaussian, 50 bins, 1e8 events per iteration, FP64, seed 0).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg4|cfg5|cfg1] [--epl E]
@@ -269,12 +269,12 @@ def run_b200(args):
              ("imad_wide", V.PIPE_IMAD_WIDE), ("lop3", V.PIPE_LOP3), ("shared_f64_add", V.PIPE_SHARED_F64_ADD))} if rank == 0 else {}
 
     def step_async():
-        if world == 1:
-            nl = g.iterate_enqueue(n, epl, w.seed)
-        else:                               # this rank's shard, ONE all-reduce of the 8 + d*N partials, S6 on every rank
-            nl = S.iterate_sharded_enqueue(g, n, epl, w.seed) + 1
-        g.refine_enqueue(w.alpha)           # S7, no host round trip; outcome collected after the timed region
-        return nl + 1                       # iterate launches (S6 runs in their last CTA) + the refine kernel
+        if world == 1:                      # the fused step: S6 and S7 run in the last CTA of the iteration's kernels,
+            return g.step_enqueue(n, epl, w.seed, w.alpha)      # no memset, no separate refine kernel, no host round trip
+        # this rank's shard, ONE all-reduce of the 8 + d*N partials, S6 (finalize kernel) and S7 on every rank
+        nl = S.iterate_sharded_enqueue(g, n, epl, w.seed) + 1
+        g.refine_enqueue(w.alpha)           # outcome collected after the timed region
+        return nl + 1
 
     # ---- device-timed region ----
     g.reset()

@@ -142,6 +142,19 @@ int vegas_refine(vegas_ctx* ctx, double alpha);
 int vegas_refine_enqueue(vegas_ctx* ctx, double alpha);
 int vegas_refine_collect(vegas_ctx* ctx);
 
+/* One whole step -- vegas_iterate_enqueue + vegas_refine_enqueue -- with the refinement FUSED into the iteration's
+ * kernels: the CTA that finishes last over all launches of the iteration runs S6 and then S7 (one warp per dimension, in
+ * the shared memory the event loop no longer needs), commits the grid and clears the accumulators, so a step is one
+ * kernel per launch and needs no memset and no separate refinement kernel (the latency of small iterations:
+ * BASELINE.json configs[0]).  Same numbers as the two calls.  Asynchronous; afterwards vegas_iterate_collect (without
+ * hist: it was consumed, and cleared even if the refinement was rejected), vegas_last_sums, vegas_last_npass and
+ * vegas_refine_collect (the refinement's outcome) work as after the two calls.  vegas_run_integration replays this step
+ * as a CUDA graph.  Falls back to the two kernels if the launch shape has less shared memory than one dimension's
+ * refinement needs.
+ * Errors: those of vegas_iterate_enqueue and vegas_refine_enqueue. */
+int vegas_step_enqueue(vegas_ctx* ctx, uint64_t n_events, uint64_t events_per_launch, uint64_t seed, double alpha,
+                       int* n_kernel_launches);
+
 /* Device time (ms, CUDA events on the context's stream: memset + launches + finalize) of the iteration enqueued
  * `back` iterations ago (0 = the latest).  The last 64 iterations keep their events.  Synchronises on that
  * iteration's end event.  VEGAS_EINVAL if `back` is out of range. */

@@ -272,8 +272,10 @@ struct vegas_ctx {
     bool last_graph;                 // the latest iteration(s) ran as graph replays of whole steps: no per-iteration events
     double last_graph_ms;            // their average device time per step
     bool shard_pending;              // vegas_iterate_shard_enqueue ran and vegas_finalize_enqueue has not yet
+    bool accum_clean;                // [partials | H | slots | pass counter | ticket] are all zero on the device (after create /
+                                     // reset and after every fused step, whose last CTA clears them): no memset needed
     cudaGraphExec_t igexec;          // captured {memset, launches} of one many-launch iteration (vegas_iterate) for the key below
-    uint64_t ig_n, ig_first, ig_count, ig_epl, ig_seed; int ig_threads, ig_ctas, ig_rshift, ig_shard, ig_launches; const Instance* ig_inst;
+    double ig_alpha; uint64_t ig_n, ig_first, ig_count, ig_epl, ig_seed; int ig_threads, ig_ctas, ig_rshift, ig_shard, ig_launches; const Instance* ig_inst;
 };
 
 namespace {
@@ -404,6 +406,12 @@ void fill_args(const vegas_ctx* c, uint64_t seed, uint64_t first, uint32_t count
         a.rk0[r] = k0 + static_cast<uint32_t>(r) * 0x9E3779B9u;
         a.rk1[r] = k1 + static_cast<uint32_t>(r) * 0xBB67AE85u;
     }
+    a.refine_alpha = -1.0;
+    a.edges = reinterpret_cast<double*>(c->ws + c->L.edges);
+    a.new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);
+    a.status = reinterpret_cast<int*>(c->ws + c->L.status);
+    a.precision = c->precision == VEGAS_FP32_EVAL ? 1 : 0;
+    a.smem_bytes = static_cast<int>(c->smem_bytes);
     a.dim = c->dim;
     a.nbins = c->nbins;
     a.rshift = c->rshift;
@@ -502,6 +510,7 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0; c->rt_lib = nullptr; c->rt_inst = nullptr;
     c->hist_consumed = false; c->last_graph = false; c->last_graph_ms = 0.0; c->shard_pending = false; c->igexec = nullptr;
+    c->accum_clean = false;
     c->n_user_params = n_params;
     int rc = setup_integrand(c, params);
     if (rc != VEGAS_OK) { delete c; return rc; }
@@ -534,6 +543,7 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     rc = build_table(c, 1);
     if (rc != VEGAS_OK) return cleanup(rc);
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return cleanup(fail(VEGAS_ECUDA, "create: %s", cudaGetErrorString(cudaGetLastError())));
+    c->accum_clean = true;                               // the whole workspace was just zeroed
     *out = c;
     return VEGAS_OK;
 }
@@ -644,14 +654,33 @@ enum IterMode {
 };
 
 static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
-                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard);
+                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard, double fuse_alpha = -1.0);
 static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
-                          uint64_t seed, int* n_kernel_launches, bool shard);
+                          uint64_t seed, int* n_kernel_launches, bool shard, double fuse_alpha = -1.0);
 
 int vegas_iterate_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed,
                           int* n_kernel_launches)
 {
     return iterate_common(c, n_events, 0, n_events, events_per_launch, seed, n_kernel_launches, false);
+}
+
+// true if the refinement of this context's grid fits in the dynamic shared memory of its iterate launches
+static bool can_fuse_refine(const vegas_ctx* c)
+{
+    return c->smem_bytes >= 4 * (static_cast<size_t>(c->nbins) + 1) * sizeof(double);
+}
+
+int vegas_step_enqueue(vegas_ctx* c, uint64_t n_events, uint64_t events_per_launch, uint64_t seed, double alpha,
+                       int* n_kernel_launches)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
+    if (can_fuse_refine(c)) return iterate_common(c, n_events, 0, n_events, events_per_launch, seed, n_kernel_launches, false, alpha);
+    // (a launch shape with less shared memory than one dimension's refinement needs: two kernels)
+    int rc = iterate_common(c, n_events, 0, n_events, events_per_launch, seed, n_kernel_launches, false);
+    if (rc == VEGAS_OK) rc = vegas_refine_enqueue(c, alpha);
+    if (rc == VEGAS_OK && n_kernel_launches) *n_kernel_launches += 1;
+    return rc;
 }
 
 int vegas_iterate_shard_enqueue(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count,
@@ -683,10 +712,10 @@ __global__ void set_u32_kernel(uint32_t* p, uint32_t v) { *p = v; }
 
 // Capture {memset, all launches} of one iteration with this geometry into a CUDA graph (kept until the key changes).
 static int ensure_iter_graph(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t epl, uint64_t seed,
-                             bool shard, int* launches)
+                             bool shard, double fuse_alpha, int* launches)
 {
     if (c->igexec && c->ig_n == n_total && c->ig_first == first && c->ig_count == count && c->ig_epl == epl &&
-        c->ig_seed == seed && c->ig_shard == (shard ? 1 : 0) && c->ig_threads == c->threads && c->ig_ctas == c->ctas_per_sm &&
+        c->ig_seed == seed && c->ig_alpha == fuse_alpha && c->ig_shard == (shard ? 1 : 0) && c->ig_threads == c->threads && c->ig_ctas == c->ctas_per_sm &&
         c->ig_rshift == c->rshift && c->ig_inst == c->inst) {
         if (launches) *launches = c->ig_launches;
         return VEGAS_OK;
@@ -697,7 +726,7 @@ static int ensure_iter_graph(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     cudaError_t e = cudaStreamBeginCapture(c->gstream, cudaStreamCaptureModeRelaxed);
     if (e != cudaSuccess) { c->stream = user; return fail(VEGAS_ECUDA, "cudaStreamBeginCapture failed: %s", cudaGetErrorString(e)); }
     int nl = 0;
-    const int rc = enqueue_iteration(c, n_total, first, count, epl, seed, &nl, kGraphIter, shard);
+    const int rc = enqueue_iteration(c, n_total, first, count, epl, seed, &nl, kGraphIter, shard, fuse_alpha);
     cudaGraph_t graph = nullptr;
     e = cudaStreamEndCapture(c->gstream, &graph);       // always leave capture mode
     c->stream = user;
@@ -707,6 +736,7 @@ static int ensure_iter_graph(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     cudaGraphDestroy(graph);
     if (e2 != cudaSuccess) { c->igexec = nullptr; return fail(VEGAS_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
     c->ig_n = n_total; c->ig_first = first; c->ig_count = count; c->ig_epl = epl; c->ig_seed = seed; c->ig_shard = shard ? 1 : 0;
+    c->ig_alpha = fuse_alpha;
     c->ig_threads = c->threads; c->ig_ctas = c->ctas_per_sm; c->ig_rshift = c->rshift; c->ig_inst = c->inst;
     c->ig_launches = nl;
     if (launches) *launches = nl;
@@ -717,7 +747,7 @@ static int ensure_iter_graph(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
 // host-side bookkeeping.  Iterations cut into many launches replay a captured graph (vegas_use_cuda_graph): the
 // host's launch rate (2-2.5 us per cudaLaunchKernel) is otherwise the floor of small batches.
 static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
-                          uint64_t seed, int* n_kernel_launches, bool shard)
+                          uint64_t seed, int* n_kernel_launches, bool shard, double fuse_alpha)
 {
     uint64_t bound = 0;
     int rc = check_iteration_args(c, n_total, first, count, events_per_launch, &bound);
@@ -726,23 +756,26 @@ static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64
     int launches = 0;
     const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
     if (c->use_graph && (count + epl - 1) / epl >= kGraphMinLaunches) {
-        rc = ensure_iter_graph(c, n_total, first, count, events_per_launch, seed, shard, &launches);
+        rc = ensure_iter_graph(c, n_total, first, count, events_per_launch, seed, shard, fuse_alpha, &launches);
         if (rc != VEGAS_OK) return rc;
         CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
         set_u32_kernel<<<1, 1, 0, c->stream>>>(reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter), c->iteration);
         CUDA_TRY(cudaGraphLaunch(c->igexec, c->stream));
     } else {
         CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
-        rc = enqueue_iteration(c, n_total, first, count, events_per_launch, seed, &launches, kPlain, shard);
+        rc = enqueue_iteration(c, n_total, first, count, events_per_launch, seed, &launches, kPlain, shard, fuse_alpha);
         if (rc != VEGAS_OK) return rc;
     }
     CUDA_TRY(cudaEventRecord(c->evB[evi], c->stream));
+    const bool fused = fuse_alpha >= 0.0;
     c->n_enqueued += 1;
     c->iteration += 1;
-    c->have_hist = !shard;                               // a shard's H is partial until the all-reduce + vegas_finalize_enqueue
-    c->have_sums = !shard;
+    c->have_hist = !shard && !fused;                     // a shard's H is partial until the all-reduce + vegas_finalize_enqueue;
+    c->have_sums = !shard;                               // a fused step's H was consumed (and cleared) by its refinement
     c->shard_pending = shard;
     c->hist_consumed = false;
+    c->accum_clean = fused;
+    if (fused) c->refine_pending += 1;
     c->last_graph = false;
     c->last_n = n_total;
     c->last_launches = launches;
@@ -753,13 +786,17 @@ static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64
 // Enqueue {memset, launches} of the events [first, first + count) of an iteration of n_total events.  Pure enqueue: no
 // timing events, no bookkeeping (iterate_common / the graph captures do that).
 static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
-                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard)
+                             uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard, double fuse_alpha)
 {
     uint64_t bound = 0;
     const int rc0 = check_iteration_args(c, n_total, first, count, events_per_launch, &bound);
     if (rc0 != VEGAS_OK) return rc0;
     const uint64_t epl = events_per_launch < (uint64_t(1) << 31) ? events_per_launch : (uint64_t(1) << 31);
-    CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    // the accumulators are cleared by one memset -- unless the previous step was a fused one, whose last CTA left them clean
+    // (a captured graph always carries the memset unless it is a fused step's: those are only replayed on clean accumulators)
+    const bool fused = fuse_alpha >= 0.0;
+    if (!(fused && (mode == kGraphStep || (mode == kPlain && c->accum_clean))))
+        CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
     if (n_kernel_launches) *n_kernel_launches = 0;
     if (count == 0) return VEGAS_OK;                     // an empty shard contributes zeros
     IterArgs a;
@@ -822,6 +859,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     a.dev_iter = (mode == kGraphStep) ? reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter) : nullptr;
     a.ring = (mode == kGraphStep) ? reinterpret_cast<double*>(c->ws + c->L.ring) : nullptr;
     a.ring_len = kRing;
+    a.refine_alpha = fused ? fuse_alpha : -1.0;
     int launches = 0;
     for (uint64_t at = first; at < last;) {
         const uint64_t cnt = launch_count(at);
@@ -937,6 +975,7 @@ int vegas_set_histogram(vegas_ctx* c, const double* hist)
     c->have_hist = true;
     c->hist_consumed = false;
     c->shard_pending = false;
+    c->accum_clean = false;
     return VEGAS_OK;
 }
 
@@ -978,6 +1017,7 @@ int vegas_refine_collect(vegas_ctx* c)
     const int pending = c->refine_pending;
     c->refine_pending = 0;
     // the latest refinement was rejected and nothing overwrote H since: the histogram is still there for another try
+    // (not after a fused step: its refinement clears H either way and sets no hist_consumed)
     if (c->h_status[2] != 0 && c->hist_consumed) { c->have_hist = true; c->hist_consumed = false; }
     if (c->h_status[0] != 0)
         return fail(VEGAS_EGRID, "refined edges were not strictly increasing in %d of the last %d refinement(s); each of those left its grid and histogram unchanged", c->h_status[0], pending);
@@ -1035,6 +1075,7 @@ int vegas_tune_events_per_launch(vegas_ctx* c, uint64_t n_events, uint64_t seed,
     c->have_sums = false;
     c->hist_consumed = false;
     c->shard_pending = false;
+    c->accum_clean = false;
     return rc;
 }
 
@@ -1079,8 +1120,15 @@ static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint
         return VEGAS_OK;
     if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
     CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
-    int rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false);
-    if (rc == VEGAS_OK) { c->have_hist = true; rc = vegas_refine_enqueue(c, alpha); }
+    // one kernel per launch, the last CTA of the iteration refines (fused step); two kernels if the launch shape has too
+    // little shared memory for that.  No memset either way: run_steps_graph_on clears the accumulators once before the
+    // first replay and every step leaves them clean.
+    int rc;
+    if (can_fuse_refine(c)) rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false, alpha);
+    else {
+        rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false);     // (carries its memset)
+        if (rc == VEGAS_OK) { c->have_hist = true; rc = vegas_refine_enqueue(c, alpha); }
+    }
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);     // always leave capture mode
     c->refine_pending = 0;
@@ -1124,6 +1172,8 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     uint32_t* h_it = reinterpret_cast<uint32_t*>(c->h_status) + 4;
     *h_it = c->iteration;
     CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.dev_iter, h_it, 4, cudaMemcpyHostToDevice, c->stream));
+    if (!c->accum_clean)                                 // the captured fused step has no memset of its own
+        CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
     double* ring = reinterpret_cast<double*>(c->ws + c->L.ring);
     stamp_kernel<<<1, 1, 0, c->stream>>>(ring + 3 * kRing);
     CUDA_TRY(cudaEventRecord(c->run_ev0, c->stream));
@@ -1152,7 +1202,8 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     c->last_graph_ms = static_cast<double>(ms) / total;
     c->iteration += static_cast<uint32_t>(total);
     c->have_hist = false;                                // the last step refined
-    c->hist_consumed = true;
+    c->hist_consumed = !can_fuse_refine(c);              // (a fused step clears H whatever the outcome)
+    c->accum_clean = can_fuse_refine(c);
     c->have_sums = true;
     c->shard_pending = false;
     c->last_n = n_events;
@@ -1254,6 +1305,7 @@ int vegas_reset(vegas_ctx* c)
     c->have_sums = false;
     c->hist_consumed = false;
     c->shard_pending = false;
+    c->accum_clean = true;
     return VEGAS_OK;
 }
 

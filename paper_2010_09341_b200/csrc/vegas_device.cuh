@@ -67,6 +67,13 @@ struct IterArgs {
     uint32_t* dev_iter;        // graph replays: advanced by S6 (NULL otherwise)
     double* ring;              // graph replays: (I, sigma) log (NULL otherwise)
     int ring_len;
+    // fused step (vegas_step_enqueue): the CTA that finishes last also refines (S7) and leaves the accumulators clean
+    double refine_alpha;       // < 0: no refinement in this kernel
+    double* edges;             // device: master edges E[dim][nbins+1]
+    double* new_edges;         // device: candidate edges
+    int* status;               // device: refinement status words (rejected count, -, latest outcome)
+    int precision;             // 0: fp64 table, 1: fp32 table
+    int smem_bytes;            // dynamic shared memory of this launch (reused by the refinement)
     uint32_t rk0[10], rk1[10];  // Philox round keys: k + r * Weyl
     int dim, nbins;
     int rshift;            // log2 of the number R of lane-indexed histogram replicas in shared memory

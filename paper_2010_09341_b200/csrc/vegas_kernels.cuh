@@ -180,6 +180,10 @@ __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, i
                                               double* partials, double* result, uint32_t* dev_iter, double* ring,
                                               int ring_len);
 
+__device__ __forceinline__ void refine_all(double* edges, double* hist, int N, double alpha, double* new_edges, int d,
+                                           void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes,
+                                           bool clear_hist_always);
+
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
 {
@@ -354,10 +358,19 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
         sh_last = (atomicAdd(a.ticket, 1u) == a.total_ctas - 1u);
     }
     __syncthreads();
-    if (sh_last && tid < 32) {
-        __threadfence();                                 // see the other CTAs' slots
+    if (!sh_last) return;
+    __threadfence();                                     // see the other CTAs' slots and histogram reductions
+    if (tid < 32)
         finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.partials, a.result,
                       a.dev_iter, a.ring, a.ring_len);
+    if (a.refine_alpha >= 0.0) {
+        // ---- fused step: S7 by the same CTA, in the shared memory the event loop no longer needs; then the
+        // accumulators are cleared, so the next step needs no memset ----
+        __syncthreads();                                 // S6 has read the slots and the pass counter
+        refine_all(a.edges, a.hist, N, a.refine_alpha, a.new_edges, d, const_cast<void*>(a.table), a.precision, a.status,
+                   smem_raw, static_cast<size_t>(a.smem_bytes), true);
+        for (int i = tid; i < a.fin_lanes * a.fin_used * 4; i += blockDim.x) a.slots0[i] = 0.0;
+        if (tid == 0) { *a.npass = 0ull; *a.ticket = 0u; }
     }
 }
 
@@ -507,8 +520,8 @@ __device__ __forceinline__ int refine_dimension_warp(const double* __restrict__ 
     const int chunk = (N + 31) >> 5;
     const int lo = lane * chunk < N ? lane * chunk : N, hi = (lo + chunk < N) ? lo + chunk : N;
 
-    for (int i = lane; i < N; i += 32) A[i] = hg[i];
-    for (int i = lane; i <= N; i += 32) E[i] = Eg[i];
+    for (int i = lane; i < N; i += 32) A[i] = __ldcg(hg + i);           // H was reduced into L2 by other CTAs
+    for (int i = lane; i <= N; i += 32) E[i] = __ldcg(Eg + i);
     __syncwarp();
     double part = 0.0;                                   // step 1
     for (int i = lo; i < hi; ++i) part = __dadd_rn(part, A[i]);
@@ -594,7 +607,8 @@ __device__ __forceinline__ int refine_dimension_warp(const double* __restrict__ 
 // refine again, e.g. with another alpha) and status[0] counts the rejection (the host clears it when it collects
 // the outcome of the refinements enqueued since); status[2] = the latest outcome.
 __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, double alpha, double* new_edges, int d,
-                                           void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes)
+                                           void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes,
+                                           bool clear_hist_always)
 {
     __shared__ int sh_bad;
     const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
@@ -618,23 +632,27 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
         if (bad) status[0] += 1;                         // refinements rejected since the host last collected
         status[2] = bad;                                 // outcome of the most recent refinement
     }
-    if (bad) return;                                     // grid, table and H stay as they were
     const int cells = d * N;
+    if (bad) {                                           // grid and table stay as they were; H too, unless this is the fused
+        if (clear_hist_always)                           // step (the next step's iteration starts from clean accumulators)
+            for (int c = threadIdx.x; c < cells; c += blockDim.x) hist[c] = 0.0;
+        return;
+    }
     for (int c = threadIdx.x; c < cells; c += blockDim.x) {
         const int k = c / N, i = c - k * N;
         const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
-        const double lo = En[i], hi = En[i + 1];
+        const double lo = __ldcg(En + i), hi = __ldcg(En + i + 1);      // written by other warps of this CTA
         write_table_cell(table, precision, static_cast<size_t>(c), lo, __dsub_rn(hi, lo));
         hist[c] = 0.0;
     }
-    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = new_edges[e];
+    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = __ldcg(new_edges + e);
 }
 
 __global__ void refine_kernel(double* edges, double* hist, int N, double alpha, double* new_edges, int d, void* table,
                               int precision, int* status, int smem_bytes)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    refine_all(edges, hist, N, alpha, new_edges, d, table, precision, status, smem_raw, static_cast<size_t>(smem_bytes));
+    refine_all(edges, hist, N, alpha, new_edges, d, table, precision, status, smem_raw, static_cast<size_t>(smem_bytes), false);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -29,6 +29,7 @@ SIGNATURES = {
     "vegas_refine": (C.c_int, [_vp, C.c_double]),
     "vegas_refine_enqueue": (C.c_int, [_vp, C.c_double]),
     "vegas_refine_collect": (C.c_int, [_vp]),
+    "vegas_step_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_double, _ip]),
     "vegas_iteration_kernel_ms": (C.c_int, [_vp, C.c_int, _dp]),
     "vegas_set_table": (C.c_int, [_vp, _dp, C.c_int]),
     "vegas_get_grid": (C.c_int, [_vp, _dp]),
@@ -181,6 +182,14 @@ class Vegas:
         epl = int(events_per_launch) if events_per_launch else n_events
         nl = C.c_int()
         _chk(lib().vegas_iterate_enqueue(self._h, n_events, epl, int(seed), C.byref(nl)), "vegas_iterate_enqueue")
+        return nl.value
+
+    def step_enqueue(self, n_events, events_per_launch=0, seed=0, alpha=1.5):
+        """One fused step (iteration + refinement in the same kernels); returns the number of kernels launched."""
+        n_events = int(n_events)
+        epl = int(events_per_launch) if events_per_launch else n_events
+        nl = C.c_int()
+        _chk(lib().vegas_step_enqueue(self._h, n_events, epl, int(seed), float(alpha), C.byref(nl)), "vegas_step_enqueue")
         return nl.value
 
     def refine_enqueue(self, alpha):

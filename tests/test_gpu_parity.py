@@ -487,6 +487,39 @@ def test_tune_events_per_launch_leaves_state_alone_and_prefers_large_batches(V, 
     assert_iteration_close(g.iterate(300_000, best, w.seed), o.iterate(300_000, w.seed, threads=THREADS))
 
 
+@pytest.mark.parametrize("name,n,epl", [("cfg1", 10**5, 0), ("cfg2", 400_003, 0), ("cfg2", 400_003, 60_000), ("cfg2", 400_003, 20_000),
+                                        ("cfg4", 300_000, 0), ("cfg5", 300_000, 100_000), ("toy_d32", 200_000, 0), ("toy_f32_d9", 200_000, 0)])
+def test_fused_step_equals_iterate_plus_refine_and_the_oracle(V, O, name, n, epl):
+    """vegas_step_enqueue (S1-S7 in one kernel per launch: the last CTA finalizes, refines, commits and clears the
+    accumulators; no memset between steps) against the oracle, five free-running steps, single launch / several launches /
+    graph-replayed many launches."""
+    w = small_workloads()[name]
+    g, o = make_pair(V, O, w)
+    for it in range(5):
+        oI, os_, _ = o.iterate(n, w.seed, threads=THREADS)
+        launches = g.step_enqueue(n, epl, w.seed, w.alpha)
+        assert launches == (1 if not epl else -(-n // epl))
+        gI, gs, _ = g.iterate_collect(want_hist=False)
+        assert abs(gI - oI) <= 1e-12 * abs(oI) and abs(gs - os_) <= 1e-12 * abs(os_), (it, gI, oI, gs, os_)
+        if o.npass is not None:
+            assert g.last_npass() == o.npass
+        with pytest.raises(V.VegasError) as ei:
+            g.iterate_collect(want_hist=True)           # consumed by the fused refinement
+        assert ei.value.code == V.ESTATE
+        o.refine(w.alpha)
+        g.refine_collect()
+        assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12, (it, np.max(np.abs(g.get_grid() - o.get_grid())))
+    # a plain iteration after fused steps starts from clean accumulators as well
+    assert_iteration_close(g.iterate(n, epl, w.seed), o.iterate(n, w.seed, threads=THREADS))
+    # ... and a fused step after a plain iteration (dirty accumulators: the memset comes back)
+    o.refine(w.alpha); g.refine(w.alpha)
+    g.step_enqueue(n, epl, w.seed, w.alpha); g.refine_collect()
+    oI, os_, _ = o.iterate(n, w.seed, threads=THREADS); o.refine(w.alpha)
+    gI, gs, _ = g.iterate_collect(want_hist=False)
+    assert abs(gI - oI) <= 1e-12 * abs(oI) and abs(gs - os_) <= 1e-12 * abs(os_)
+    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
+
+
 def test_async_step_equals_blocking_step(V):
     """vegas_iterate_enqueue + vegas_refine_enqueue (bench.py's device-timed step) against the blocking calls."""
     w = W.cfg1()
