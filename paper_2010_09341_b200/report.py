@@ -20,6 +20,8 @@ from . import workloads as W
 
 def run_config(name, w, n_iter=None, epl=0, tune=False):
     g = V.from_workload(w)
+    if w.integrand_id == W.LO_2TO2_TAB:
+        g.set_table(W.pdf_table())
     n_iter = n_iter or w.n_iter
     g.iterate(w.n_events, epl, w.seed)          # untimed warm-up on the uniform grid
     tuned = None
