@@ -184,6 +184,71 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
                                            void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes,
                                            bool clear_hist_always);
 
+// What every CTA of an iterate launch does after its events: the CTA's compensated sums go to its slot, the replicas of
+// its `cells` histogram cells (global cells cell0 ...) are summed and reduced into H, and the CTA that finishes last
+// over all launches of the iteration runs S6 -- and, in a fused step, S7.
+__device__ __forceinline__ void cta_tail(const IterArgs& a, Comp s1, Comp s2, unsigned int np, const double* sh_hist,
+                                         double* sh_part, int cells, int cell0, int rs, int d, int N, unsigned char* smem_raw)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int R = 1 << rs;
+    // ---- scalar sums: warp shuffle tree on compensated pairs, then one thread per CTA ----
+    comp_warp_reduce(s1);
+    comp_warp_reduce(s2);
+    np = __reduce_add_sync(0xFFFFFFFFu, np);
+    const int warp = tid >> 5, nwarps = (blockDim.x + 31) >> 5;
+    if (lane == 0) {
+        sh_part[warp * 5 + 0] = s1.hi; sh_part[warp * 5 + 1] = s1.lo;
+        sh_part[warp * 5 + 2] = s2.hi; sh_part[warp * 5 + 3] = s2.lo;
+        sh_part[warp * 5 + 4] = static_cast<double>(np);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        // the CTA's slot carries over from the previous launches of this iteration (stream order)
+        double* slot = a.slots + static_cast<size_t>(blockIdx.x) * 4;
+        Comp t1{slot[0], slot[1]}, t2{slot[2], slot[3]};
+        unsigned long long npb = 0;
+        for (int w = 0; w < nwarps; ++w) {
+            comp_add(t1, sh_part[w * 5 + 0], sh_part[w * 5 + 1]);
+            comp_add(t2, sh_part[w * 5 + 2], sh_part[w * 5 + 3]);
+            npb += static_cast<unsigned long long>(sh_part[w * 5 + 4]);
+        }
+        slot[0] = t1.hi; slot[1] = t1.lo; slot[2] = t2.hi; slot[3] = t2.lo;
+        if (npb) atomicAdd(a.npass, npb);
+    }
+
+    // ---- histogram flush: fixed-order sum over the replicas, one global reduction per touched cell ----
+    for (int c = tid; c < cells; c += blockDim.x) {
+        const double* p = sh_hist + (static_cast<size_t>(c) << rs);
+        double v = p[c & (R - 1)];                              // rotated start: conflict-free reads
+        for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[(r + c) & (R - 1)]);
+        if (v != 0.0) atomicAdd(a.hist + cell0 + c, v);
+    }
+
+    // ---- S6 in the CTA that finishes last over all launches of this iteration ----
+    __shared__ int sh_last;
+    __syncthreads();                                     // this CTA's slot is written
+    if (tid == 0) {
+        __threadfence();
+        sh_last = (atomicAdd(a.ticket, 1u) == a.total_ctas - 1u);
+    }
+    __syncthreads();
+    if (!sh_last) return;
+    __threadfence();                                     // see the other CTAs' slots and histogram reductions
+    if (tid < 32)
+        finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.partials, a.result,
+                      a.dev_iter, a.ring, a.ring_len);
+    if (a.refine_alpha >= 0.0) {
+        // ---- fused step: S7 by the same CTA, in the shared memory the event loop no longer needs; then the
+        // accumulators are cleared, so the next step needs no memset ----
+        __syncthreads();                                 // S6 has read the slots and the pass counter
+        refine_all(a.edges, a.hist, N, a.refine_alpha, a.new_edges, d, const_cast<void*>(a.table), a.precision, a.status,
+                   smem_raw, static_cast<size_t>(a.smem_bytes), true);
+        for (int i = tid; i < a.fin_lanes * a.fin_used * 4; i += blockDim.x) a.slots0[i] = 0.0;
+        if (tid == 0) { *a.npass = 0ull; *a.ticket = 0u; }
+    }
+}
+
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_constant__ IterArgs a)
 {
@@ -317,61 +382,7 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
         if (lane < qn) consume((head + lane) & (kQueueCap - 1));
     }
 
-    // ---- scalar sums: warp shuffle tree on compensated pairs, then one thread per CTA ----
-    comp_warp_reduce(s1);
-    comp_warp_reduce(s2);
-    np = __reduce_add_sync(0xFFFFFFFFu, np);
-    const int warp = tid >> 5, nwarps = (blockDim.x + 31) >> 5;
-    if (lane == 0) {
-        sh_part[warp * 5 + 0] = s1.hi; sh_part[warp * 5 + 1] = s1.lo;
-        sh_part[warp * 5 + 2] = s2.hi; sh_part[warp * 5 + 3] = s2.lo;
-        sh_part[warp * 5 + 4] = static_cast<double>(np);
-    }
-    __syncthreads();
-    if (tid == 0) {
-        // the CTA's slot carries over from the previous launches of this iteration (stream order)
-        double* slot = a.slots + static_cast<size_t>(blockIdx.x) * 4;
-        Comp t1{slot[0], slot[1]}, t2{slot[2], slot[3]};
-        unsigned long long npb = 0;
-        for (int w = 0; w < nwarps; ++w) {
-            comp_add(t1, sh_part[w * 5 + 0], sh_part[w * 5 + 1]);
-            comp_add(t2, sh_part[w * 5 + 2], sh_part[w * 5 + 3]);
-            npb += static_cast<unsigned long long>(sh_part[w * 5 + 4]);
-        }
-        slot[0] = t1.hi; slot[1] = t1.lo; slot[2] = t2.hi; slot[3] = t2.lo;
-        if (npb) atomicAdd(a.npass, npb);
-    }
-
-    // ---- histogram flush: fixed-order sum over the replicas, one global reduction per touched cell ----
-    for (int c = tid; c < cells; c += blockDim.x) {
-        const double* p = sh_hist + (static_cast<size_t>(c) << rs);
-        double v = p[c & (R - 1)];                              // rotated start: conflict-free reads
-        for (int r = 1; r < R; ++r) v = __dadd_rn(v, p[(r + c) & (R - 1)]);
-        if (v != 0.0) atomicAdd(a.hist + c, v);
-    }
-
-    // ---- S6 in the CTA that finishes last over all launches of this iteration ----
-    __shared__ int sh_last;
-    __syncthreads();                                     // this CTA's slot is written
-    if (tid == 0) {
-        __threadfence();
-        sh_last = (atomicAdd(a.ticket, 1u) == a.total_ctas - 1u);
-    }
-    __syncthreads();
-    if (!sh_last) return;
-    __threadfence();                                     // see the other CTAs' slots and histogram reductions
-    if (tid < 32)
-        finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.partials, a.result,
-                      a.dev_iter, a.ring, a.ring_len);
-    if (a.refine_alpha >= 0.0) {
-        // ---- fused step: S7 by the same CTA, in the shared memory the event loop no longer needs; then the
-        // accumulators are cleared, so the next step needs no memset ----
-        __syncthreads();                                 // S6 has read the slots and the pass counter
-        refine_all(a.edges, a.hist, N, a.refine_alpha, a.new_edges, d, const_cast<void*>(a.table), a.precision, a.status,
-                   smem_raw, static_cast<size_t>(a.smem_bytes), true);
-        for (int i = tid; i < a.fin_lanes * a.fin_used * 4; i += blockDim.x) a.slots0[i] = 0.0;
-        if (tid == 0) { *a.npass = 0ull; *a.ticket = 0u; }
-    }
+    cta_tail(a, s1, s2, np, sh_hist, sh_part, cells, 0, rs, d, N, smem_raw);
 }
 
 // ------------------------------------------------------------------------------------------------
