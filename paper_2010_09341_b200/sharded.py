@@ -43,3 +43,26 @@ def iterate_sharded_enqueue(ctx, n_events: int, events_per_launch: int = 0, seed
         dist.all_reduce(ctx.partials_tensor(), op=dist.ReduceOp.SUM, group=group)   # the iteration's one exchange
     ctx.finalize_enqueue(int(n_events))
     return launches
+
+
+def run_integration_sharded(ctx, n_iter: int, n_events: int, events_per_launch: int = 0, seed: int = 0, alpha: float = 1.5,
+                            n_warmup: int = 0, group=None):
+    """PAPER.md:L79 `run_integration` over the ranks of a process group (the paper's multi-GPU mode, L53-L57):
+    (n_warmup + n_iter) x {sharded iteration, identical refinement on every rank}, then the classic inverse-variance
+    combination of the last n_iter iterations (the library's host routine vegas_combine_iterations).  Every rank returns
+    the same (mean, error, chi2_dof, {integral, error}); one all-reduce per iteration is the only communication.  A
+    refinement rejected for a non-monotone grid leaves the grid unchanged on every rank alike and the run goes on."""
+    import numpy as np
+    from . import vegas as V
+    total = int(n_iter) + int(n_warmup)
+    I, s = np.empty(total), np.empty(total)
+    for it in range(total):
+        iterate_sharded_enqueue(ctx, n_events, events_per_launch, seed, group=group)
+        I[it], s[it], _ = ctx.iterate_collect(want_hist=False)
+        try:
+            ctx.refine(alpha)
+        except V.VegasError as e:
+            if e.code != V.EGRID:
+                raise
+    mean, err, chi2 = V.combine_iterations(I[n_warmup:], s[n_warmup:])
+    return mean, err, chi2, dict(integral=I, error=s)

@@ -129,3 +129,17 @@ def test_shard_argument_errors(V):
     g.finalize_enqueue(1000)
     I, s, h = g.iterate_collect()
     assert I == 0.0 and s == 0.0 and not h.any()
+
+
+@pytest.mark.gpu
+def test_run_integration_sharded_equals_the_library_driver_without_a_process_group(V):
+    """Without a process group the sharded driver is the whole range on one rank: same estimates as
+    vegas_run_integration (plain loop and graph replay)."""
+    w = W.cfg1()
+    a, b = V.from_workload(w), V.from_workload(w)
+    m1, e1, c1, log1 = sharded.run_integration_sharded(a, 4, 50_000, 0, w.seed, w.alpha, n_warmup=2)
+    m2, e2, c2, log2 = b.run_integration(4, 50_000, 0, w.seed, w.alpha, n_warmup=2)
+    np.testing.assert_allclose(log1["integral"], log2["integral"], rtol=1e-12)
+    np.testing.assert_allclose(log1["error"], log2["error"], rtol=1e-11)
+    assert abs(m1 - m2) <= 1e-12 * abs(m2) and abs(e1 - e2) <= 1e-11 * e2 and abs(c1 - c2) <= 1e-8 * max(c2, 1e-30)
+    np.testing.assert_allclose(a.get_grid(), b.get_grid(), rtol=0, atol=1e-12)
