@@ -285,6 +285,7 @@ namespace {
 int setup_integrand(vegas_ctx* c, const double* p)
 {
     std::memset(&c->ic, 0, sizeof(c->ic));
+    fill_exp_consts(c->ic.ec);
     switch (c->integrand_id) {
         case VEGAS_GAUSS_SYM:
         case VEGAS_GAUSS_DOUBLE: {

@@ -42,7 +42,25 @@ struct IntegrandConsts {
     // lo_2to2_tab: the tabulated PDF (device pointer into the workspace, vegas_set_table) and its length
     const double* tab;
     int ntab;
+    // exp_f64: log2(e), 1.5 * 2^52, -ln2 (high, low), 1/13! ... 1/2!  (kernel parameters, so that every use is a
+    // uniform-register operand of the fused multiply-add and costs neither a register nor a move)
+    double ec[16];
 };
+
+#ifndef __CUDACC_RTC__
+// The table behind IntegrandConsts::ec, filled by the host (vegas_api.cu).
+inline void fill_exp_consts(double* ec)
+{
+    ec[0] = 0x1.71547652b82fep+0;            // log2(e), rounded
+    ec[1] = 0x1.8p52;                        // 1.5 * 2^52: adding it leaves round(x log2 e) in the low word
+    ec[2] = -0x1.62e42fefa39efp-1;           // -rnd(ln 2)
+    ec[3] = -0x1.abc9e3b39803fp-56;          // -rnd(ln 2 - rnd(ln 2))
+    double f = 1.0;
+    for (int n = 2; n <= 13; ++n) f *= static_cast<double>(n);      // 13! = 6227020800, exact
+    for (int n = 13; n >= 2; --n) { ec[4 + (13 - n)] = 1.0 / f; f /= static_cast<double>(n); }   // 1/n!: one rounding each
+}
+#endif
+
 
 constexpr int kMaxUserParams = 16;
 
@@ -83,18 +101,12 @@ struct IterArgs {
 // ------------------------------------------------------------------------------------------------
 // S1 -- Philox4x32-10 (Salmon et al. 2011): multipliers 0xD2511F53 / 0xCD9E8D57, ten rounds, round
 // function (hi(M1 c2)^c1^k0, lo(M1 c2), hi(M0 c0)^c3^k1, lo(M0 c0)).  Round keys come precomputed.
-// VEGAS_PHILOX_MULHI selects hi/lo by two instructions (IMAD.HI + IMAD) instead of one IMAD.WIDE.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void mulhilo(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo)
 {
-#ifdef VEGAS_PHILOX_MULHI
-    hi = __umulhi(a, b);
-    lo = a * b;
-#else
-    const uint64_t p = static_cast<uint64_t>(a) * static_cast<uint64_t>(b);
+    const uint64_t p = static_cast<uint64_t>(a) * static_cast<uint64_t>(b);      // one IMAD.WIDE.U32
     hi = static_cast<uint32_t>(p >> 32);
     lo = static_cast<uint32_t>(p);
-#endif
 }
 
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
@@ -176,6 +188,49 @@ __device__ __forceinline__ void ldg_cell(const void* table, int cell, float& lo,
 }
 
 // ------------------------------------------------------------------------------------------------
+// exp for the built-in fp64 integrands: k = round(x log2 e) by the 1.5 * 2^52 shift, r = x - k ln 2 in two fused
+// steps (ln 2 split in a rounded part and its remainder), e^r by the degree-13 Taylor polynomial (|r| <= 0.347:
+// remainder 6e-18 relative), scaled by 2^k through the exponent field.  Within about one unit in the last place of
+// the correctly rounded value (the tests allow 2e-15 relative against the oracle's libm).  Every constant is a
+// kernel parameter: on sm_100a a DFMA with three register operands takes three issue cycles, one with two registers
+// and a uniform operand under two (measured), and CUDA's exp() rebuilds its thirteen constants
+// in registers with two moves each.  Outside |x| < 700 (overflow, subnormal results) the library routine is used.
+// ------------------------------------------------------------------------------------------------
+template <int NX>
+__device__ __forceinline__ void exp_f64(const double (&x)[NX], double (&y)[NX], const IntegrandConsts& c)
+{
+    bool in_range = true;
+#pragma unroll
+    for (int j = 0; j < NX; ++j) in_range = in_range && (fabs(x[j]) < 700.0);
+    if (!in_range) {
+#pragma unroll
+        for (int j = 0; j < NX; ++j) y[j] = exp(x[j]);
+        return;
+    }
+    // the NX evaluations run side by side: one load of each constant, NX independent chains
+    int k[NX];
+    double r[NX], p[NX];
+#pragma unroll
+    for (int j = 0; j < NX; ++j) {
+        const double t = __fma_rn(x[j], c.ec[0], c.ec[1]);
+        k[j] = __double2loint(t);
+        const double kf = __dsub_rn(t, c.ec[1]);
+        r[j] = __fma_rn(kf, c.ec[3], __fma_rn(kf, c.ec[2], x[j]));
+        p[j] = c.ec[4];
+    }
+#pragma unroll
+    for (int i = 5; i < 16; ++i)
+#pragma unroll
+        for (int j = 0; j < NX; ++j) p[j] = __fma_rn(p[j], r[j], c.ec[i]);
+#pragma unroll
+    for (int j = 0; j < NX; ++j) {
+        p[j] = __fma_rn(p[j], r[j], 1.0);
+        p[j] = __fma_rn(p[j], r[j], 1.0);
+        y[j] = __hiloint2double(__double2hiint(p[j]) + (k[j] << 20), __double2loint(p[j]));
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // S3 -- integrands as streaming accumulators: begin(), coord(k, x_k) in ascending k, end() -> f.
 // Evaluation order is the normative one of SURVEY.md 8.c I0-I4; every fused multiply-add is explicit
 // and every other product/sum uses the non-contracting intrinsics.
@@ -195,7 +250,10 @@ struct GaussSym {            // I0, BASELINE.json configs[0]
     __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
     __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
     {
-        return __dmul_rn(c.gC, exp(-__dmul_rn(s, c.ga2)));
+        const double x[1] = {-__dmul_rn(s, c.ga2)};
+        double e[1];
+        exp_f64(x, e, c);
+        return __dmul_rn(c.gC, e[0]);
     }
 };
 
@@ -215,9 +273,10 @@ struct GaussDouble {         // I1, BASELINE.json configs[1], [2]
     __device__ __forceinline__ bool precheck(const IntegrandConsts&) const { return true; }
     __device__ __forceinline__ double end(const IntegrandConsts& c, int) const
     {
-        const double e1 = exp(-__dmul_rn(s1, c.ga2));
-        const double e2 = exp(-__dmul_rn(s2, c.ga2));
-        return __dmul_rn(c.ghalfC, __dadd_rn(e1, e2));        // ghalfC = fl(0.5*C) (exact), set by the host
+        const double x[2] = {-__dmul_rn(s1, c.ga2), -__dmul_rn(s2, c.ga2)};
+        double e[2];
+        exp_f64(x, e, c);
+        return __dmul_rn(c.ghalfC, __dadd_rn(e[0], e[1]));        // ghalfC = fl(0.5*C) (exact), set by the host
     }
 };
 
@@ -295,9 +354,10 @@ struct Lo2to2 {              // I3, BASELINE.json configs[4], dim = 3: (v1, v2, 
         const double v1 = v[0], v2 = v[1], v3 = v[2];
         const double L = c.hL;
         const double cth = __fma_rn(2.0, v3, -1.0);
-        const double x1 = exp(__dmul_rn(v1, L));
-        const double x2 = exp(__dmul_rn(v2, L));
-        const double e12 = exp(__dmul_rn(-c.ha, __dmul_rn(__dadd_rn(v1, v2), L)));   // x1^-a x2^-a
+        const double ax[3] = {__dmul_rn(v1, L), __dmul_rn(v2, L), __dmul_rn(-c.ha, __dmul_rn(__dadd_rn(v1, v2), L))};
+        double ex[3];
+        exp_f64(ax, ex, c);
+        const double x1 = ex[0], x2 = ex[1], e12 = ex[2];                                  // e12 = x1^-a x2^-a
         const double y12 = __dmul_rn(__dsub_rn(1.0, x1), __dsub_rn(1.0, x2));
         const double y2 = __dmul_rn(y12, y12);
         const double y5 = __dmul_rn(__dmul_rn(y2, y2), y12);                              // ((1-x1)(1-x2))^5

@@ -112,6 +112,26 @@ def test_events_adapted_grid(V, O, name):
         assert np.any(o.events(0, 100, w.seed)["jac"] != 1.0)
 
 
+@pytest.mark.parametrize("alpha", [0.3, 0.05, 0.02])
+def test_events_exp_ranges(V, O, alpha):
+    """The kernels' own exp (exp_f64: |argument| < 700) and the library routine it hands over to beyond that, against
+    the oracle's libm: narrow Gaussians drive the arguments of exp from 0 down past -708 (subnormal results) to total
+    underflow.  Normal results agree to 2e-15 relative, subnormal ones to one unit of the subnormal grid."""
+    for wl in (W.Workload("gs_exp", 4, 50, W.GAUSS_SYM, (alpha, 0.5), W.FP64, 10**5, 1),
+               W.Workload("gd_exp", 8, 50, W.GAUSS_DOUBLE, (alpha, 1 / 3, 2 / 3), W.FP64, 10**5, 1)):
+        g, o = make_pair(V, O, wl)
+        eg, eo = g.debug_events(0, 50_000, seed=3), o.events(0, 50_000, 3)
+        np.testing.assert_array_equal(eg["x"], eo["x"])
+        fg, fo = eg["f"], eo["f"]
+        normal = fo >= 1e-290
+        np.testing.assert_allclose(fg[normal], fo[normal], rtol=2e-15, atol=0.0)
+        np.testing.assert_allclose(fg[~normal], fo[~normal], rtol=0.0, atol=1e-290 * 2e-15)
+        if alpha == 0.02:
+            assert np.any(fo == 0.0) and np.any(normal)     # both regimes are present
+        n = 200_003
+        assert_iteration_close(g.iterate(n, 0, 3), o.iterate(n, 3, threads=THREADS))
+
+
 # ---------------------------------------------------------------------------------------------------
 # one iteration (S1-S6): several tiles + a ragged tail, several launch splits
 # ---------------------------------------------------------------------------------------------------
