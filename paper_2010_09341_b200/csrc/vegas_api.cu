@@ -24,8 +24,10 @@ using namespace vegas;
 constexpr int kMaxTable = 4096;         // doubles of integrand data (tabulated PDF)
 constexpr int kRing = 64;               // (I, sigma) entries logged on the device between two reads of a graph run
 constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
-constexpr int kLanes = 32;              // internal streams the launches of one iteration are dealt to (a8): 8 of them, all 32
-                                        // when there are so many launches that each gets 1/8 of the SMs or less
+constexpr int kLanes = 128;             // internal streams the launches of one iteration are dealt to (a8): as many as the
+                                        // device runs kernels concurrently
+constexpr double kCtaOverheadEvents = 3.0;   // a CTA's prologue + flush + launch cost, in events per thread (measured on
+                                        // configs[1]: ~6 us against 2.2 us per event and thread of a full SM)
 constexpr int kLaneSlots = 2048;        // upper bound on the iterate grid (CTAs) = slots of a lane's region
 constexpr int kMaxSlots = 8 * kLaneSlots;   // lanes x (largest grid among the launches) never exceeds this
 constexpr size_t kStaticSmemReserve = 1024;   // the opt-in shared-memory limit covers static + dynamic: room for the kernels' few static words
@@ -809,13 +811,27 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     // several launches they are dealt round-robin to kLanes internal streams forked from the caller's stream:
     // launches that do not fill the GPU overlap, and every launch's prologue/flush overlaps its neighbours'.
     const uint64_t n_launches = (count + epl - 1) / epl;
-    const int lanes = n_launches >= 64 ? kLanes : n_launches > 1 ? 8 : 1;
-    // several launches in flight: each takes a fraction of the SMs, so that one launch's prologue / flush overlaps
-    // its neighbours' event loops (a CTA of a tuned instance fills an SM's shared memory: full-size grids cannot
-    // share an SM).  The fraction grows with the number of launches (measured on cfg3: 2.03 / 2.16 / 3.11 ms per
-    // 1e8 events at 1e7 / 1e6 / 1e5 events per launch with 1/2, 1/4, 1/8 of the SMs, against 2.06 / 2.52 / 5.83).
-    const int split = n_launches >= 512 ? 8 : n_launches >= 32 ? 4 : n_launches >= 8 ? 2 : 1;
-    const int cap_grid = (max_grid + split - 1) / split;
+    // Launch geometry of a many-launch iteration (configs[2]): every launch gets the same grid g, chosen by a wave model.
+    // With L launches of cnt events each, up to min(L, kLanes) of them in flight and S CTA slots on the device,
+    // the CTAs run in ceil(L g / min(S, lanes g)) waves, each as long as one CTA: its fixed cost (zeroing and flushing
+    // the shared histogram, staging the table, the launch itself: kCtaOverheadEvents events per thread) plus
+    // cnt / (g threads) events per thread.  Small g amortises the fixed cost, large g evens out the last wave; the model
+    // reproduces the measured times of the batch-size sweep to a few percent.
+    int lanes = 1, cap_grid = max_grid;
+    if (n_launches > 1) {
+        const double L = static_cast<double>(n_launches);
+        const int lanes_max = n_launches < static_cast<uint64_t>(kLanes) ? static_cast<int>(n_launches) : kLanes;
+        const double per_thread = static_cast<double>(epl < count ? epl : count) / static_cast<double>(c->threads);
+        double best = 0.0;
+        for (int g = 1; g <= max_grid; ++g) {
+            const double conc = std::fmin(static_cast<double>(max_grid), static_cast<double>(lanes_max) * g);
+            const double waves = std::ceil(L * g / conc);
+            const double cost = waves * (kCtaOverheadEvents + per_thread / g);
+            if (g == 1 || cost < best * (1.0 - 1e-9)) { best = cost; cap_grid = g; }
+        }
+        lanes = lanes_max;
+        while (lanes > 1 && static_cast<size_t>(lanes) * cap_grid > static_cast<size_t>(kMaxSlots)) --lanes;
+    }
     if (lanes > 1) {
         CUDA_TRY(cudaEventRecord(c->fork, c->stream));
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
@@ -830,11 +846,8 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
         const uint64_t to_wrap = (uint64_t(1) << 32) - (at & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
         return cnt > to_wrap ? to_wrap : cnt;
     };
-    // a CTA's prologue and flush (zero and sum R replicas of d*N cells) cost as much as several grid-strides of events:
-    // when many small launches share the GPU each gets fewer CTAs with at least kMinStrides events per thread
-    const uint64_t kMinStrides = n_launches >= 8 ? 4 : 1;
-    auto launch_grid = [&](uint64_t cnt) {
-        uint64_t want = (cnt + static_cast<uint64_t>(c->threads) * kMinStrides - 1) / (static_cast<uint64_t>(c->threads) * kMinStrides);
+    auto launch_grid = [&](uint64_t cnt) {               // never more threads than events
+        uint64_t want = (cnt + static_cast<uint64_t>(c->threads) - 1) / static_cast<uint64_t>(c->threads);
         if (want < 1) want = 1;
         return want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
     };
@@ -851,8 +864,8 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     a.ticket = reinterpret_cast<unsigned int*>(c->ws + c->L.npass) + 4;   // inside the region cleared by the memset
     a.total_ctas = static_cast<unsigned int>(total_ctas);
     a.slots0 = slots0;
-    // slot regions: one per stream lane, used_grid slots each (lanes x used_grid <= kMaxSlots: 32 lanes are only used
-    // with grids of at most 1/8 of the SMs x CTAs per SM <= kLaneSlots / 8)
+    // slot regions: one per stream lane, used_grid slots each (lanes x used_grid <= kMaxSlots: the lane count was
+    // reduced above if the wave model picked a grid too large for that)
     if (static_cast<size_t>(lanes) * used_grid > static_cast<size_t>(kMaxSlots)) return fail(VEGAS_EINVAL, "launch geometry needs more slot regions than the workspace holds");
     a.fin_lanes = lanes; a.fin_stride = used_grid; a.fin_used = used_grid;
     a.n_events = shard ? 0ull : n_total;

@@ -405,9 +405,9 @@ def test_full_size_cascade(V, O, name):
 
 def test_cfg3_sweep_parity(V, O):
     """BASELINE.json configs[2]: 1e8 events of the d=8 double Gaussian split into launches of 1e4 ... 1e8 events; every
-    split is compared with ONE oracle iteration (not with another GPU run).  10 000 / 1 000 launches run on 1/8 of the
-    SMs each over 8 internal streams (as a replayed CUDA graph, and for 1e4 / 1e5 also as plain launches), 100 on 1/4,
-    10 on 1/2, 1 on all."""
+    split is compared with ONE oracle iteration (not with another GPU run).  The launches are dealt to up to 128 internal
+    streams with the grid the library's wave model picks (10 000 launches of one CTA each, 1 000 of two, 100 of about
+    sixteen, 10 of half the SMs, 1 of all), as a replayed CUDA graph and, for 1e4 / 1e5, also as plain launches."""
     w = W.cfg3()
     g, o = make_pair(V, O, w)
     ores = o.iterate(w.n_events, w.seed, threads=THREADS)
@@ -473,8 +473,8 @@ def test_state_after_graph_run_set_grid_and_consumed_histogram(V):
 
 def test_batch_size_study_shape(V):
     """configs[2] / PAPER.md:L65: throughput suffers when the batch is too small and reaches a plateau.
-    Loose, timing-based: 1e4-event launches (1000 of them, replayed as a CUDA graph over 32 internal streams) are at
-    least 1.5x slower per event than 1e7-event launches, and 1e6-event launches are within a factor 2.5 of them."""
+    Loose, timing-based: 1e4-event launches (1000 of them, replayed as a CUDA graph over 128 internal streams) are at
+    least 1.2x slower per event than 1e7-event launches, and 1e6-event launches are within a factor 2.5 of them."""
     w = W.cfg2(n_events=10**7)
     g = V.from_workload(w)
     ms = {}
@@ -486,7 +486,7 @@ def test_batch_size_study_shape(V):
             g.iterate(w.n_events, epl, w.seed, want_hist=False)
             best = min(best, g.last_sums()[2])
         ms[epl] = best
-    assert ms[10**4] > 1.5 * ms[10**7], ms
+    assert ms[10**4] > 1.2 * ms[10**7], ms
     assert ms[10**6] >= 0.95 * ms[10**7] and ms[10**6] < 2.5 * ms[10**7], ms
 
 
