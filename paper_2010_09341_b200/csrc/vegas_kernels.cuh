@@ -203,18 +203,26 @@ __device__ __forceinline__ void cta_tail(const IterArgs& a, Comp s1, Comp s2, un
         sh_part[warp * 5 + 4] = static_cast<double>(np);
     }
     __syncthreads();
-    if (tid == 0) {
-        // the CTA's slot carries over from the previous launches of this iteration (stream order)
-        double* slot = a.slots + static_cast<size_t>(blockIdx.x) * 4;
-        Comp t1{slot[0], slot[1]}, t2{slot[2], slot[3]};
-        unsigned long long npb = 0;
-        for (int w = 0; w < nwarps; ++w) {
-            comp_add(t1, sh_part[w * 5 + 0], sh_part[w * 5 + 1]);
-            comp_add(t2, sh_part[w * 5 + 2], sh_part[w * 5 + 3]);
-            npb += static_cast<unsigned long long>(sh_part[w * 5 + 4]);
+    if (warp == 0) {
+        // the warps' partial sums (at most 32) go through the same compensated shuffle tree, then into the CTA's slot,
+        // which carries over from the previous launches of this iteration (stream order)
+        Comp t1{0.0, 0.0}, t2{0.0, 0.0};
+        unsigned int npw = 0u;
+        if (lane < nwarps) {
+            t1.hi = sh_part[lane * 5 + 0]; t1.lo = sh_part[lane * 5 + 1];
+            t2.hi = sh_part[lane * 5 + 2]; t2.lo = sh_part[lane * 5 + 3];
+            npw = static_cast<unsigned int>(sh_part[lane * 5 + 4]);
         }
-        slot[0] = t1.hi; slot[1] = t1.lo; slot[2] = t2.hi; slot[3] = t2.lo;
-        if (npb) atomicAdd(a.npass, npb);
+        comp_warp_reduce(t1);
+        comp_warp_reduce(t2);
+        const unsigned int npb = __reduce_add_sync(0xFFFFFFFFu, npw);     // <= 32 * 2^26 events of one launch per CTA: no overflow
+        if (lane == 0) {
+            double* slot = a.slots + static_cast<size_t>(blockIdx.x) * 4;
+            comp_add(t1, slot[0], slot[1]);
+            comp_add(t2, slot[2], slot[3]);
+            slot[0] = t1.hi; slot[1] = t1.lo; slot[2] = t2.hi; slot[3] = t2.lo;
+            if (npb) atomicAdd(a.npass, static_cast<unsigned long long>(npb));
+        }
     }
 
     // ---- histogram flush: fixed-order sum over the replicas, one global reduction per touched cell ----

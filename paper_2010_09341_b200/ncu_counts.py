@@ -1,6 +1,6 @@
 """Per-event instruction counts and DRAM traffic of the iterate kernel, read from an ncu report.
 
-    python -m paper_2010_09341_b200.ncu_counts <report.ncu-rep> <workload> <n_events> [--md] [--launch K]
+    python -m paper_2010_09341_b200.ncu_counts <report.ncu-rep> <workload> <n_events> [--md | --summary] [--launch K]
 
 Reads the report with `ncu -i <report> --page raw --csv` (whole-launch counters) and `--page source --csv` (executed
 count of every SASS instruction; needs --import-source at capture time and -lineinfo at compile time) and prints ONE
@@ -11,8 +11,10 @@ csv row: what one launch executed, divided by the events it processed --
 `inst` .. `atoms` are warp instructions x 32 / n_events = thread instructions per event (retries of lost histogram races
 included, predicated-off lanes counted: these are issue slots and pipe cycles, which is what bounds the kernel).
 bench.py reads the committed table (profiles/r02_kernel_counts.csv) for the co-bounds of its roofline block and for
-`roofline.traffic`; `--md` prints the opcode histogram as a markdown table instead (profiles/r02_sass_hist_*.md).
-No GPU needed: ncu only parses the report.
+`roofline.traffic`; `--md` prints the opcode histogram as a markdown table instead (profiles/r02_sass_hist_*.md);
+`--summary` prints the whole-launch counters the design discussion quotes (pipes, issue slots, shared-memory
+wavefronts and bank conflicts, DRAM bytes, stall reasons per issued instruction) as a markdown table
+(profiles/r02_ncu_full_*.md).  No GPU needed: ncu only parses the report.
 """
 from __future__ import annotations
 
@@ -25,6 +27,46 @@ import sys
 FP64 = ("DADD", "DFMA", "DMUL", "DSETP")
 FP32 = ("FADD", "FFMA", "FMUL", "FSETP", "FSEL", "FMNMX", "FCHK", "MUFU")
 HEADER = "workload,kernel,n_events,kernel_us,dram_bytes,inst,fp64,fp32,imad_wide,imad,lop3,lds,atoms"
+SUMMARY = """Kernel Name
+gpu__time_duration.sum
+launch__registers_per_thread
+launch__shared_mem_per_block_dynamic
+launch__block_size
+launch__grid_size
+smsp__inst_executed.sum
+smsp__issue_active.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active
+sm__pipe_fmaheavy_cycles_active.avg.pct_of_peak_sustained_elapsed
+sm__pipe_fma_cycles_active.avg.pct_of_peak_sustained_active
+sm__pipe_alu_cycles_active.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_xu.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_cbu.avg.pct_of_peak_sustained_active
+sm__inst_executed_pipe_adu.avg.pct_of_peak_sustained_active
+l1tex__data_pipe_lsu_wavefronts_mem_shared.sum
+l1tex__data_pipe_lsu_wavefronts_mem_shared.sum.pct_of_peak_sustained_elapsed
+l1tex__data_pipe_lsu_wavefronts_mem_shared_op_atom.sum
+l1tex__data_pipe_lsu_wavefronts_mem_shared_op_ld.sum
+l1tex__data_pipe_lsu_wavefronts_mem_shared_op_st.sum
+l1tex__data_bank_conflicts_pipe_lsu_mem_shared_op_ld.sum
+l1tex__data_bank_conflicts_pipe_lsu_mem_shared_op_atom.sum
+smsp__inst_executed_op_shared_atom.sum
+smsp__sass_inst_executed_op_shared_ld.sum
+smsp__sass_inst_executed_op_shared_st.sum
+dram__bytes_read.sum
+dram__bytes_write.sum
+sm__warps_active.avg.pct_of_peak_sustained_active
+sm__throughput.avg.pct_of_peak_sustained_elapsed
+sm__cycles_elapsed.avg
+sm__cycles_elapsed.avg.per_second
+smsp__thread_inst_executed_per_inst_executed.ratio
+smsp__thread_inst_executed_pred_on_per_inst_executed.ratio""".splitlines()
+STALL = "smsp__average_warps_issue_stalled_%s_per_issue_active.ratio"
+STALLS = ("barrier", "branch_resolving", "dispatch_stall", "drain", "lg_throttle", "long_scoreboard", "math_pipe_throttle",
+          "membar", "mio_throttle", "misc", "no_instruction", "not_selected", "selected", "short_scoreboard", "sleeping",
+          "tex_throttle", "wait")
 
 
 def _page(report, page):
@@ -70,6 +112,19 @@ def main(argv):
     raw = raw_counters(report, launch)
     cnt = opcode_counts(report)
     per = 32.0 / n
+    if "--summary" in argv:
+        units = dict(zip(_page(report, "raw")[0], _page(report, "raw")[1]))
+        print("`stall_*` = smsp__average_warps_issue_stalled_*_per_issue_active.ratio.\n\n| metric | unit | value |\n|---|---|---|")
+        for m in SUMMARY:
+            if m in raw:
+                v = raw[m]
+                if m == "Kernel Name":
+                    v = re.sub(r"\(int\)|\(bool\)|vegas::", "", v)
+                print("| %s | %s | %s |" % (m, units.get(m, ""), v))
+        for st in STALLS:
+            if STALL % st in raw:
+                print("| stall_%s | %s | %s |" % (st, units.get(STALL % st, ""), raw[STALL % st]))
+        return 0
     if "--md" in argv:
         total = sum(cnt.values())
         print("| opcode | warp instructions executed | thread instructions per event | share |\n|---|---|---|---|")
