@@ -295,9 +295,15 @@ int vegas_tune_events_per_launch(vegas_ctx* ctx, uint64_t n_events, uint64_t see
  *   VEGAS_PIPE_SHARED_F64_ADD_R8     the same update in the layout configs[3] is forced into (2000 cells, R = 8)
  *   VEGAS_PIPE_SHARED_F64_RMW_PLAIN  the non-atomic LDS.64, DADD, STS.64 a lane-and-warp-private word would allow
  *   VEGAS_PIPE_SHARED_U32_ADD        the native 32-bit integer shared-memory atomic add
+ * and, as evidence for what the event loop's issue rate is bound by (same section):
+ *   VEGAS_PIPE_DFMA_3REG             DFMA whose three source operands are three different registers (VEGAS_PIPE_DFMA
+ *                                    repeats one; a polynomial step with its coefficient in a register is this form)
+ *   VEGAS_PIPE_MIX_EVENT_LOOP        the event loop's ratio: 3 (IMAD.WIDE + LOP3), 2 IMAD, 5 DFMA, 5 LOP3 per group
+ *                                    (the rate counts all 18 instructions of a group)
  * Errors: VEGAS_EINVAL (unknown pipe, NULL out), VEGAS_ECUDA. */
 enum { VEGAS_PIPE_DFMA = 0, VEGAS_PIPE_FFMA = 1, VEGAS_PIPE_IMAD_WIDE = 2, VEGAS_PIPE_LOP3 = 3, VEGAS_PIPE_SHARED_F64_ADD = 4,
-       VEGAS_PIPE_SHARED_F64_ADD_R8 = 5, VEGAS_PIPE_SHARED_F64_RMW_PLAIN = 6, VEGAS_PIPE_SHARED_U32_ADD = 7 };
+       VEGAS_PIPE_SHARED_F64_ADD_R8 = 5, VEGAS_PIPE_SHARED_F64_RMW_PLAIN = 6, VEGAS_PIPE_SHARED_U32_ADD = 7,
+       VEGAS_PIPE_DFMA_3REG = 8, VEGAS_PIPE_MIX_EVENT_LOOP = 9 };
 int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr_per_s);
 
 #ifdef __cplusplus

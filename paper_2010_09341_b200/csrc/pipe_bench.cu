@@ -20,13 +20,15 @@ __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long 
 {
     extern __shared__ double sh[];                     // KIND 4, 6, 7: [32 cells][32 lanes]; KIND 5: [2000 cells][8 replicas]
     const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
-    double d[kChains];
+    double d[kChains], e3[kChains], g3[kChains];
     float f[kChains];
     unsigned long long w[kChains];
     uint32_t u[kChains], v[kChains];
 #pragma unroll
     for (int c = 0; c < kChains; ++c) {
         d[c] = 1.0 + 1e-9 * (t + c);
+        e3[c] = 1.0 + 1e-12 * (t + 3 * c);              // KIND 8: per-thread register operands
+        g3[c] = 1e-9 * (t + c + 1);
         f[c] = 1.0f + 1e-6f * (t + c);
         w[c] = static_cast<unsigned long long>(t * 7u + c) * 0x9E3779B97F4A7C15ull + seed;
         u[c] = t * 31u + c + seed;
@@ -66,6 +68,18 @@ __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long 
                     double* p = &sh[((u[c] >> 27) << 5) + (threadIdx.x & 31)];
                     asm volatile("{\n\t.reg .f64 t;\n\tld.volatile.f64 t, [%0];\n\tadd.rn.f64 t, t, %1;\n\tst.volatile.f64 [%0], t;\n\t}" :: "l"(p), "d"(db) : "memory");
                 }
+                if (KIND == 8)      // DFMA with three distinct register operands (a Horner step whose coefficient is in a register)
+                    asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(d[c]) : "d"(e3[c]), "d"(g3[c]));
+                if (KIND == 9) {   // the event loop's ratio: 3 (IMAD.WIDE + LOP3) Philox half-rounds, 2 IMAD, 5 fp64, 5 LOP3
+                    if (c < 3) {
+                        const uint32_t x = static_cast<uint32_t>(w[c] >> 32) ^ static_cast<uint32_t>(w[c]) ^ seed;
+                        asm volatile("mul.wide.u32 %0, %1, %2;" : "=l"(w[c]) : "r"(x), "r"(0xD2511F53u));
+                    }
+                    if (c >= 3 && c < 5) asm volatile("mad.lo.u32 %0, %0, %1, %1;" : "+r"(u[c]) : "r"(seed));
+                    if (c < 5) asm volatile("fma.rn.f64 %0, %0, %1, %1;" : "+d"(d[c]) : "d"(e3[c]));
+                    // logic operations chained across the chains (u[c] with its neighbour), so that none can be merged
+                    if (c >= 3) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(u[c]) : "r"(u[c == 7 ? 3 : c + 1]), "r"(seed));
+                }
                 if (KIND == 7) {
                     // the native shared-memory atomic: 32-bit integer add (cannot hold the histogram's dynamic range)
                     u[c] = u[c] * 1664525u + 1013904223u;
@@ -77,7 +91,8 @@ __global__ void __launch_bounds__(1024, 1) pipe_kernel(int iters, unsigned long 
     unsigned long long acc = 0;
 #pragma unroll
     for (int c = 0; c < kChains; ++c)
-        acc += static_cast<unsigned long long>(__double_as_longlong(d[c])) + __float_as_uint(f[c]) + w[c] + u[c] + v[c];
+        acc += static_cast<unsigned long long>(__double_as_longlong(d[c])) + __float_as_uint(f[c]) + w[c] + u[c] + v[c] +
+               static_cast<unsigned long long>(__double_as_longlong(e3[c])) + static_cast<unsigned long long>(__double_as_longlong(g3[c]));
     if (acc == 0x1234567ull) out[t] = acc;             // never true in practice: keeps the chains alive
 }
 
@@ -105,7 +120,9 @@ cudaError_t time_kind(int sms, int iters, unsigned long long* out, cudaStream_t 
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     if (e != cudaSuccess) return e;
-    const double ops = static_cast<double>(iters) * kUnroll * kChains * blocks * threads;
+    // instructions per pass over the chains: one per chain, except the mixed group of KIND 9 (18)
+    const double per_pass = (KIND == 9) ? 18.0 : static_cast<double>(kChains);
+    const double ops = static_cast<double>(iters) * kUnroll * per_pass * blocks * threads;
     *rate = ops / (best * 1e-3);
     return cudaSuccess;
 }
@@ -133,6 +150,8 @@ extern "C" int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr
         case VEGAS_PIPE_SHARED_F64_ADD_R8: e = time_kind<5>(sms, 50, out, st, thread_instr_per_s); break;
         case VEGAS_PIPE_SHARED_F64_RMW_PLAIN: e = time_kind<6>(sms, 100, out, st, thread_instr_per_s); break;
         case VEGAS_PIPE_SHARED_U32_ADD: e = time_kind<7>(sms, 100, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_DFMA_3REG: e = time_kind<8>(sms, 500, out, st, thread_instr_per_s); break;
+        case VEGAS_PIPE_MIX_EVENT_LOOP: e = time_kind<9>(sms, 500, out, st, thread_instr_per_s); break;
         default: cudaFree(out); return VEGAS_EINVAL;
     }
     cudaFree(out);

@@ -65,7 +65,8 @@ def main():
                                            ("lop3", V.PIPE_LOP3), ("shared_f64_add", V.PIPE_SHARED_F64_ADD),
                                            ("shared_f64_add_r8", V.PIPE_SHARED_F64_ADD_R8),
                                            ("shared_f64_rmw_plain", V.PIPE_SHARED_F64_RMW_PLAIN),
-                                           ("shared_u32_add", V.PIPE_SHARED_U32_ADD))}
+                                           ("shared_u32_add", V.PIPE_SHARED_U32_ADD), ("dfma_3reg", V.PIPE_DFMA_3REG),
+                                           ("mix_event_loop", V.PIPE_MIX_EVENT_LOOP))}
     print(json.dumps({"pipe_rates_thread_instr_per_s": pipes}))
     for name in args.configs.split(","):
         w = W.ALL[name]()
