@@ -999,9 +999,12 @@ int vegas_refine_enqueue(vegas_ctx* c, double alpha)
     if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
     if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
     const int N = c->nbins;
-    // one warp per dimension, all in one CTA; as many dimensions at a time as fit in shared memory
+    // all dimensions in one CTA, as many at a time as fit in shared memory (at most one per warp); the steps that are
+    // independent per bin use ceil((N + 1) / 32) warps per dimension when the CTA has them
     const size_t per_dim = 4 * (static_cast<size_t>(N) + 1) * sizeof(double);
     const int warps = c->dim < 32 ? c->dim : 32;
+    int cta_warps = warps * ((N + 1 + 31) / 32);
+    if (cta_warps > 32) cta_warps = 32;
     const size_t max_smem = static_cast<size_t>(c->smem_optin) - kStaticSmemReserve;
     size_t smem = per_dim * static_cast<size_t>(warps);
     if (smem > max_smem) smem = (max_smem / per_dim) * per_dim;
@@ -1011,7 +1014,7 @@ int vegas_refine_enqueue(vegas_ctx* c, double alpha)
     double* new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);
     double* hist = reinterpret_cast<double*>(c->ws + c->L.hist);
     int* status = reinterpret_cast<int*>(c->ws + c->L.status);
-    refine_kernel<<<1, 32 * warps, smem, c->stream>>>(edges, hist, N, alpha, new_edges, c->dim, c->ws + c->L.table,
+    refine_kernel<<<1, 32 * cta_warps, smem, c->stream>>>(edges, hist, N, alpha, new_edges, c->dim, c->ws + c->L.table,
                                                       c->precision == VEGAS_FP32_EVAL ? 1 : 0, status, static_cast<int>(smem));
     CUDA_TRY(cudaGetLastError());
     c->have_hist = false;

@@ -500,7 +500,7 @@ __global__ void build_table_kernel(double* __restrict__ edges, void* __restrict_
     }
 }
 
-// S7 (refine): one warp per dimension, all dimensions in ONE CTA, so that the all-or-nothing commit of step 7 needs
+// S7 (refine): all dimensions in ONE CTA, so that the all-or-nothing commit of step 7 needs
 // no grid-wide dependency.  The refinement is latency-bound (d*N <= a few thousand cells, chains of dependent fp64
 // operations at ~40 cycles each), so everything that the definition states as a sequential sum is done as a
 // lane-chunked sum / scan instead: lane l owns the contiguous bins [l*chunk, (l+1)*chunk), sums or scans them locally
@@ -527,48 +527,23 @@ __device__ __forceinline__ double damp_pow(double x, double alpha)
     return pow(x, alpha);
 }
 
-// returns 1 if this dimension's new edges are not strictly increasing, else 0 (same value in every lane)
-__device__ __forceinline__ int refine_dimension_warp(const double* __restrict__ Eg, const double* __restrict__ hg, int N,
-                                                     double alpha, double* __restrict__ Eng, double* sm)
+// The warp-level pieces of S7 for one dimension (called by the warp that owns the dimension; lane l owns the
+// contiguous bins [lo, hi)).  Each returns its result in every lane.
+__device__ __forceinline__ double refine_chunk_sum(const double* v, int lo, int hi)
+{
+    double part = 0.0;
+    for (int i = lo; i < hi; ++i) part = __dadd_rn(part, v[i]);
+    return warp_sum_all(part);
+}
+
+// steps 5: prefix sums cum[1..N] of m[0..N-1] (chunk-local prefix, scan of the 32 chunk totals, exact max-scan so that
+// the prefix sums never decrease across a chunk boundary), cum[0] = 0.  Returns cum[N].
+__device__ __forceinline__ double refine_prefix(const double* m, double* cum, int N, int lo, int hi)
 {
     const int lane = threadIdx.x & 31;
-    double* A = sm;                                      // [N+1] h, then m
-    double* B = A + (N + 1);                             // [N+1] s, then new edges
-    double* cum = B + (N + 1);                           // [N+1]
-    double* E = cum + (N + 1);                           // [N+1]
-    const int chunk = (N + 31) >> 5;
-    const int lo = lane * chunk < N ? lane * chunk : N, hi = (lo + chunk < N) ? lo + chunk : N;
-
-    for (int i = lane; i < N; i += 32) A[i] = __ldcg(hg + i);           // H was reduced into L2 by other CTAs
-    for (int i = lane; i <= N; i += 32) E[i] = __ldcg(Eg + i);
-    __syncwarp();
-    double part = 0.0;                                   // step 1
-    for (int i = lo; i < hi; ++i) part = __dadd_rn(part, A[i]);
-    const double tot = warp_sum_all(part);
-    if (!(tot > 0.0) || !isfinite(tot)) {                // nothing to adapt to: dimension unchanged
-        for (int i = lane; i <= N; i += 32) Eng[i] = E[i];
-        return 0;
-    }
-    part = 0.0;                                          // steps 2 + 3
+    double part = 0.0;
     for (int i = lo; i < hi; ++i) {
-        double v;
-        if (i == 0) v = __ddiv_rn(__dadd_rn(A[0], A[1]), 2.0);
-        else if (i == N - 1) v = __ddiv_rn(__dadd_rn(A[N - 2], A[N - 1]), 2.0);
-        else v = __ddiv_rn(__dadd_rn(__dadd_rn(A[i - 1], A[i]), A[i + 1]), 3.0);
-        B[i] = v;
-        part = __dadd_rn(part, v);
-    }
-    const double ssum = warp_sum_all(part);
-    __syncwarp();                                        // every lane is done reading h before it becomes m
-    part = 0.0;                                          // steps 4 + 5: damped weights and their chunk-local prefix sums
-    for (int i = lo; i < hi; ++i) {
-        const double r = __ddiv_rn(B[i], ssum);
-        double v;
-        if (r <= 0.0) v = 0.0;
-        else if (r >= 1.0) v = 1.0;
-        else v = damp_pow(__ddiv_rn(__dsub_rn(1.0, r), -log(r)), alpha);
-        A[i] = v;
-        part = __dadd_rn(part, v);
+        part = __dadd_rn(part, m[i]);
         cum[i + 1] = part;                               // chunk-local for now
     }
     double incl = part;                                  // inclusive scan of the 32 chunk totals
@@ -596,56 +571,120 @@ __device__ __forceinline__ int refine_dimension_warp(const double* __restrict__ 
     }
     if (lane == 0) cum[0] = 0.0;
     __syncwarp();
-    const double delta = __ddiv_rn(cum[N], static_cast<double>(N));
-    for (int j = lane; j <= N; j += 32) {                // step 6
-        double v;
-        if (j == 0) v = 0.0;
-        else if (j == N) v = 1.0;
-        else {
-            const double t = __dmul_rn(static_cast<double>(j), delta);
-            int a = 0, b = N - 1;                        // smallest i in [0, N-1] with cum[i+1] >= t, else N-1
-            while (a < b) {
-                const int mid = (a + b) >> 1;
-                if (cum[mid + 1] >= t) b = mid; else a = mid + 1;
-            }
-            v = __dadd_rn(E[a], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[a]), A[a]), __dsub_rn(E[a + 1], E[a])));
-        }
-        B[j] = v;
-        Eng[j] = v;
-    }
-    __syncwarp();
-    int bad = 0;                                         // step 7 check
-    for (int j = lane; j < N; j += 32)
-        if (!(B[j] < B[j + 1])) bad = 1;
-    return __any_sync(0xFFFFFFFFu, bad) ? 1 : 0;
+    return cum[N];
 }
 
-// All of S7 by one CTA: candidate edges of every dimension (a warp each, in passes of as many dimensions as fit in
-// `smem_bytes` of shared memory), then step 7 for all dimensions: if every one passed, the candidate edges become
-// the master edges, the table is rebuilt and H is cleared; otherwise nothing changes (H included, so the caller may
-// refine again, e.g. with another alpha) and status[0] counts the rejection (the host clears it when it collects
-// the outcome of the refinements enqueued since); status[2] = the latest outcome.
+// All of S7 by one CTA, in passes of as many dimensions as fit in `smem_bytes` of shared memory (at most one per warp).
+// The sums and scans of a dimension are done by ONE warp (lane-chunked, so that their order depends on N only); the
+// steps that are independent per bin or per edge -- smoothing (2), damping (4: a division, a logarithm, a division and
+// a power per bin), the search and interpolation of the new edges (6) and the check (7) -- are spread over all the
+// warps the CTA has per dimension (cfg1 in the fused step: 8 warps for 50 bins), with a block barrier between the
+// steps: the refinement is a chain of dependent fp64 operations at ~40 cycles each, and this shortens the chain.
+// Then step 7 for all dimensions: if every one passed, the candidate edges become the master edges, the table is
+// rebuilt and H is cleared; otherwise nothing changes (H included, so the caller may refine again, e.g. with another
+// alpha) and status[0] counts the rejection (the host clears it when it collects the outcome of the refinements
+// enqueued since); status[2] = the latest outcome.
 __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, double alpha, double* new_edges, int d,
                                            void* table, int precision, int* status, unsigned char* smem, size_t smem_bytes,
                                            bool clear_hist_always)
 {
     __shared__ int sh_bad;
-    const int warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    __shared__ int sh_skip[kMaxDim];                     // the dimension has nothing to adapt to: edges unchanged
+    __shared__ double sh_ssum[kMaxDim], sh_delta[kMaxDim];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const size_t per_dim = 4 * (static_cast<size_t>(N) + 1);            // doubles
     int group = static_cast<int>(smem_bytes / (per_dim * sizeof(double)));
     if (group > nwarps) group = nwarps;
-    if (threadIdx.x == 0) sh_bad = 0;
+    if (group > kMaxDim) group = kMaxDim;
+    const int chunk = (N + 31) >> 5;
+    const int lo = lane * chunk < N ? lane * chunk : N, hi = (lo + chunk < N) ? lo + chunk : N;
+    if (tid == 0) sh_bad = 0;
     __syncthreads();
     for (int k0 = 0; k0 < d; k0 += group) {
-        const int k = k0 + warp;
-        if (warp < group && k < d) {
-            const int bad = refine_dimension_warp(edges + static_cast<size_t>(k) * (N + 1), hist + static_cast<size_t>(k) * N, N, alpha,
-                                                  new_edges + static_cast<size_t>(k) * (N + 1),
-                                                  reinterpret_cast<double*>(smem) + static_cast<size_t>(warp) * per_dim);
-            if (bad && (threadIdx.x & 31) == 0) sh_bad = 1;
+        const int nd = (d - k0 < group) ? d - k0 : group;
+        const int wpd = nwarps / nd;                     // warps per dimension in the element-wise steps (>= 1)
+        const int kk = warp / wpd;                       // this thread's dimension in those steps (>= nd: idle)
+        const int e0 = (warp - kk * wpd) * 32 + lane, estride = wpd * 32;
+        double* sm = reinterpret_cast<double*>(smem);
+        double* A = sm + static_cast<size_t>(kk < nd ? kk : 0) * per_dim;   // [N+1] h, then m
+        double* B = A + (N + 1);                         // [N+1] s, then the new edges
+        double* cum = B + (N + 1);                       // [N+1]
+        double* E = cum + (N + 1);                       // [N+1]
+        const bool active = kk < nd;
+        const int k = k0 + kk;
+        if (active) {                                    // H was reduced into L2 by other CTAs
+            for (int i = e0; i < N; i += estride) A[i] = __ldcg(hist + static_cast<size_t>(k) * N + i);
+            for (int i = e0; i <= N; i += estride) E[i] = __ldcg(edges + static_cast<size_t>(k) * (N + 1) + i);
         }
+        __syncthreads();
+        if (warp < nd) {                                 // step 1, by the warp that owns dimension k0 + warp
+            const double tot = refine_chunk_sum(sm + static_cast<size_t>(warp) * per_dim, lo, hi);
+            if (lane == 0) sh_skip[warp] = (!(tot > 0.0) || !isfinite(tot)) ? 1 : 0;
+        }
+        __syncthreads();
+        const bool skip = active && sh_skip[kk] != 0;
+        if (active && !skip)                             // step 2
+            for (int i = e0; i < N; i += estride) {
+                double v;
+                if (i == 0) v = __ddiv_rn(__dadd_rn(A[0], A[1]), 2.0);
+                else if (i == N - 1) v = __ddiv_rn(__dadd_rn(A[N - 2], A[N - 1]), 2.0);
+                else v = __ddiv_rn(__dadd_rn(__dadd_rn(A[i - 1], A[i]), A[i + 1]), 3.0);
+                B[i] = v;
+            }
+        __syncthreads();
+        if (warp < nd && !sh_skip[warp]) {               // step 3
+            const double ssum = refine_chunk_sum(sm + static_cast<size_t>(warp) * per_dim + (N + 1), lo, hi);
+            if (lane == 0) sh_ssum[warp] = ssum;
+        }
+        __syncthreads();                                 // every thread is done reading h before it becomes m
+        if (active && !skip) {                           // step 4: damped weights
+            const double ssum = sh_ssum[kk];
+            for (int i = e0; i < N; i += estride) {
+                const double r = __ddiv_rn(B[i], ssum);
+                double v;
+                if (r <= 0.0) v = 0.0;
+                else if (r >= 1.0) v = 1.0;
+                else v = damp_pow(__ddiv_rn(__dsub_rn(1.0, r), -log(r)), alpha);
+                A[i] = v;
+            }
+        }
+        __syncthreads();
+        if (warp < nd && !sh_skip[warp]) {               // step 5
+            double* Aw = sm + static_cast<size_t>(warp) * per_dim;
+            const double total = refine_prefix(Aw, Aw + 2 * (N + 1), N, lo, hi);
+            if (lane == 0) sh_delta[warp] = __ddiv_rn(total, static_cast<double>(N));
+        }
+        __syncthreads();
+        if (active) {                                    // step 6: the new edges
+            double* Eng = new_edges + static_cast<size_t>(k) * (N + 1);
+            const double delta = skip ? 0.0 : sh_delta[kk];
+            for (int j = e0; j <= N; j += estride) {
+                double v;
+                if (skip) v = E[j];
+                else if (j == 0) v = 0.0;
+                else if (j == N) v = 1.0;
+                else {
+                    const double t = __dmul_rn(static_cast<double>(j), delta);
+                    int a = 0, b = N - 1;                // smallest i in [0, N-1] with cum[i+1] >= t, else N-1
+                    while (a < b) {
+                        const int mid = (a + b) >> 1;
+                        if (cum[mid + 1] >= t) b = mid; else a = mid + 1;
+                    }
+                    v = __dadd_rn(E[a], __dmul_rn(__ddiv_rn(__dsub_rn(t, cum[a]), A[a]), __dsub_rn(E[a + 1], E[a])));
+                }
+                B[j] = v;
+                Eng[j] = v;
+            }
+        }
+        __syncthreads();
+        if (active && !skip) {                           // step 7 check
+            int bad = 0;
+            for (int j = e0; j < N; j += estride)
+                if (!(B[j] < B[j + 1])) bad = 1;
+            if (bad) sh_bad = 1;
+        }
+        __syncthreads();                                 // the shared arrays are reused by the next pass
     }
-    __syncthreads();                                     // every dimension's candidate edges (global) and verdict are written
     const int bad = sh_bad;
     if (threadIdx.x == 0) {
         if (bad) status[0] += 1;                         // refinements rejected since the host last collected
@@ -660,8 +699,8 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
     for (int c = threadIdx.x; c < cells; c += blockDim.x) {
         const int k = c / N, i = c - k * N;
         const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
-        const double lo = __ldcg(En + i), hi = __ldcg(En + i + 1);      // written by other warps of this CTA
-        write_table_cell(table, precision, static_cast<size_t>(c), lo, __dsub_rn(hi, lo));
+        const double lo_e = __ldcg(En + i), hi_e = __ldcg(En + i + 1);  // written by other warps of this CTA
+        write_table_cell(table, precision, static_cast<size_t>(c), lo_e, __dsub_rn(hi_e, lo_e));
         hist[c] = 0.0;
     }
     for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = __ldcg(new_edges + e);
