@@ -846,8 +846,11 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
         const uint64_t to_wrap = (uint64_t(1) << 32) - (at & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
         return cnt > to_wrap ? to_wrap : cnt;
     };
-    auto launch_grid = [&](uint64_t cnt) {               // never more threads than events
-        uint64_t want = (cnt + static_cast<uint64_t>(c->threads) - 1) / static_cast<uint64_t>(c->threads);
+    auto launch_grid = [&](uint64_t cnt) {
+        // one launch: spread even few events over all SMs (the CTAs' fixed costs run side by side; at least a warp of
+        // events each); several launches share the GPU: never more threads than events
+        const uint64_t per_cta = (n_launches == 1) ? 32u : static_cast<uint64_t>(c->threads);
+        uint64_t want = (cnt + per_cta - 1) / per_cta;
         if (want < 1) want = 1;
         return want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
     };

@@ -612,18 +612,19 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
         double* E = cum + (N + 1);                       // [N+1]
         const bool active = kk < nd;
         const int k = k0 + kk;
+        // the sums and scans of dimension kk belong to the LAST warp of its group, which has the fewest (mostly no) bins
+        // in the element-wise steps
+        const int own = (active && warp - kk * wpd == wpd - 1) ? kk : -1;
         if (active) {                                    // H was reduced into L2 by other CTAs
             for (int i = e0; i < N; i += estride) A[i] = __ldcg(hist + static_cast<size_t>(k) * N + i);
             for (int i = e0; i <= N; i += estride) E[i] = __ldcg(edges + static_cast<size_t>(k) * (N + 1) + i);
         }
         __syncthreads();
-        if (warp < nd) {                                 // step 1, by the warp that owns dimension k0 + warp
-            const double tot = refine_chunk_sum(sm + static_cast<size_t>(warp) * per_dim, lo, hi);
-            if (lane == 0) sh_skip[warp] = (!(tot > 0.0) || !isfinite(tot)) ? 1 : 0;
+        if (own >= 0) {                                  // step 1, by the warp that owns the dimension
+            const double tot = refine_chunk_sum(A, lo, hi);
+            if (lane == 0) sh_skip[own] = (!(tot > 0.0) || !isfinite(tot)) ? 1 : 0;
         }
-        __syncthreads();
-        const bool skip = active && sh_skip[kk] != 0;
-        if (active && !skip)                             // step 2
+        if (active)                                      // step 2 at the same time: it does not depend on the total
             for (int i = e0; i < N; i += estride) {
                 double v;
                 if (i == 0) v = __ddiv_rn(__dadd_rn(A[0], A[1]), 2.0);
@@ -632,9 +633,10 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
                 B[i] = v;
             }
         __syncthreads();
-        if (warp < nd && !sh_skip[warp]) {               // step 3
-            const double ssum = refine_chunk_sum(sm + static_cast<size_t>(warp) * per_dim + (N + 1), lo, hi);
-            if (lane == 0) sh_ssum[warp] = ssum;
+        const bool skip = active && sh_skip[kk] != 0;
+        if (own >= 0 && !skip) {                         // step 3
+            const double ssum = refine_chunk_sum(B, lo, hi);
+            if (lane == 0) sh_ssum[own] = ssum;
         }
         __syncthreads();                                 // every thread is done reading h before it becomes m
         if (active && !skip) {                           // step 4: damped weights
@@ -649,10 +651,9 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
             }
         }
         __syncthreads();
-        if (warp < nd && !sh_skip[warp]) {               // step 5
-            double* Aw = sm + static_cast<size_t>(warp) * per_dim;
-            const double total = refine_prefix(Aw, Aw + 2 * (N + 1), N, lo, hi);
-            if (lane == 0) sh_delta[warp] = __ddiv_rn(total, static_cast<double>(N));
+        if (own >= 0 && !skip) {                         // step 5
+            const double total = refine_prefix(A, cum, N, lo, hi);
+            if (lane == 0) sh_delta[own] = __ddiv_rn(total, static_cast<double>(N));
         }
         __syncthreads();
         if (active) {                                    // step 6: the new edges
@@ -696,14 +697,20 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
             for (int c = threadIdx.x; c < cells; c += blockDim.x) hist[c] = 0.0;
         return;
     }
+    const bool one_pass = d <= group;                    // every dimension's new edges are still in shared memory (B)
+    const double* smd = reinterpret_cast<const double*>(smem);
     for (int c = threadIdx.x; c < cells; c += blockDim.x) {
         const int k = c / N, i = c - k * N;
-        const double* En = new_edges + static_cast<size_t>(k) * (N + 1);
-        const double lo_e = __ldcg(En + i), hi_e = __ldcg(En + i + 1);  // written by other warps of this CTA
+        const double* En = one_pass ? smd + static_cast<size_t>(k) * per_dim + (N + 1) : new_edges + static_cast<size_t>(k) * (N + 1);
+        const double lo_e = one_pass ? En[i] : __ldcg(En + i);          // written by other warps of this CTA
+        const double hi_e = one_pass ? En[i + 1] : __ldcg(En + i + 1);
         write_table_cell(table, precision, static_cast<size_t>(c), lo_e, __dsub_rn(hi_e, lo_e));
         hist[c] = 0.0;
     }
-    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) edges[e] = __ldcg(new_edges + e);
+    for (int e = threadIdx.x; e < d * (N + 1); e += blockDim.x) {
+        const int k = e / (N + 1), j = e - k * (N + 1);
+        edges[e] = one_pass ? smd[static_cast<size_t>(k) * per_dim + (N + 1) + j] : __ldcg(new_edges + e);
+    }
 }
 
 __global__ void refine_kernel(double* edges, double* hist, int N, double alpha, double* new_edges, int d, void* table,
