@@ -143,7 +143,7 @@ int vegas_refine_enqueue(vegas_ctx* ctx, double alpha);
 int vegas_refine_collect(vegas_ctx* ctx);
 
 /* One whole step -- vegas_iterate_enqueue + vegas_refine_enqueue -- with the refinement FUSED into the iteration's
- * kernels: the CTA that finishes last over all launches of the iteration runs S6 and then S7 (one warp per dimension, in
+ * kernels: the CTA that finishes last over all launches of the iteration runs S6 and then S7 (all its warps, in
  * the shared memory the event loop no longer needs), commits the grid and clears the accumulators, so a step is one
  * kernel per launch and needs no memset and no separate refinement kernel (the latency of small iterations:
  * BASELINE.json configs[0]).  Same numbers as the two calls.  Asynchronous; afterwards vegas_iterate_collect (without
