@@ -383,13 +383,14 @@ def test_full_size_iteration_parity(V, O, name):
 
 @pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
 def test_full_size_cascade(V, O, name):
-    """BASELINE.json acceptance at the stated sizes: 5 free-running iterations of 1e8 events (the GPU grid is never
-    re-seeded from the oracle), refine after each.  I, sigma rel 1e-12, every H cell rel 1e-10, the pass count exact in
-    every iteration; refined edges within 1e-12 (absolute) of the oracle's after every refinement, the fifth included."""
+    """BASELINE.json acceptance at the stated sizes: the configuration's 10 free-running iterations of 1e8 events (the
+    GPU grid is never re-seeded from the oracle), refine after each.  I, sigma rel 1e-12, every H cell rel 1e-10, the
+    pass count exact in every iteration; refined edges within 1e-12 (absolute) of the oracle's after every refinement:
+    the fifth, which the acceptance names, and all the way to the tenth."""
     w = small_workloads()[name]
-    assert w.n_events == 10**8
+    assert w.n_events == 10**8 and w.n_iter == 10
     g, o = make_pair(V, O, w)
-    for it in range(5):
+    for it in range(w.n_iter):
         ores = o.iterate(w.n_events, w.seed, threads=THREADS)
         gres = g.iterate(w.n_events, 0, w.seed)
         assert_iteration_close(gres, ores)
@@ -400,7 +401,7 @@ def test_full_size_cascade(V, O, name):
         ge, oe = g.get_grid(), o.get_grid()
         assert np.all(np.diff(ge, axis=1) > 0) and np.all(ge[:, 0] == 0) and np.all(ge[:, -1] == 1)
         assert np.max(np.abs(ge - oe)) <= 1e-12, (it, np.max(np.abs(ge - oe)))
-    assert g.iteration == o.iteration == 5
+    assert g.iteration == o.iteration == w.n_iter
 
 
 def test_cfg3_sweep_parity(V, O):
