@@ -259,7 +259,9 @@ int vegas_device_info(const vegas_ctx* ctx, int* sm_count, int* sm_clock_khz);
  * replayed (the iteration counter then lives in device memory and the per-iteration (I, sigma) are logged on the
  * device together with a device time stamp; one host synchronisation per 64 iterations; iter_kernel_ms[i] is the
  * device time from the end of iteration i-1 -- for the first one, from the start of the run -- to the end of
- * iteration i, i.e. refinement i-1 + iteration i, read from %globaltimer).  vegas_use_cuda_graph(ctx, 0) selects the
+ * iteration i, i.e. refinement i-1 + iteration i, read from %globaltimer).  Steps of one launch each are captured 16 to
+ * a graph, their kernels linked by programmatic dependent launch (the next step's launch and shared-memory prologue run
+ * under this step's tail; VEGAS_NO_PDL=1 in the environment switches that off).  vegas_use_cuda_graph(ctx, 0) selects the
  * plain loop of blocking calls (per-iteration times from CUDA events, refinement excluded) and also keeps
  * vegas_iterate from replaying graphs of many-launch iterations.  Both give the same numbers.
  * Errors: VEGAS_EINVAL (n_iter < 1, n_warmup < 0, NULL mean/error, iterate's argument errors), VEGAS_ECUDA. */

@@ -23,6 +23,7 @@ using namespace vegas;
 
 constexpr int kMaxTable = 4096;         // doubles of integrand data (tabulated PDF)
 constexpr int kRing = 64;               // (I, sigma) entries logged on the device between two reads of a graph run
+constexpr int kStepsPerGraph = 16;      // consecutive single-launch steps captured into one CUDA graph (vegas_run_integration)
 constexpr int kEvPool = 64;             // CUDA-event pairs kept for the most recent iterations' device times
 constexpr int kLanes = 128;             // internal streams the launches of one iteration are dealt to (a8): as many as the
                                         // device runs kernels concurrently
@@ -109,12 +110,25 @@ struct Instance {
     const void* rt_debug;            // instead of the four function pointers above
 };
 
+// VEGAS_NO_PDL=1 in the environment switches programmatic dependent launch off (plain stream order)
+const bool g_use_pdl = [] { const char* e = std::getenv("VEGAS_NO_PDL"); return !(e && e[0] == '1'); }();
+
 // One interface for compiled-in and run-time compiled instances.
 cudaError_t inst_launch(const Instance* in, const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
 {
     if (!in->rt_iterate) return in->launch(a, grid, threads, smem, st);
     void* args[] = {const_cast<IterArgs*>(&a)};
-    return cudaLaunchKernel(in->rt_iterate, dim3(grid), dim3(threads), args, smem, st);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid));
+    cfg.blockDim = dim3(static_cast<unsigned>(threads));
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    return cudaLaunchKernelExC(&cfg, in->rt_iterate, args);
 }
 cudaError_t inst_debug(const Instance* in, const IterArgs& a, int grid, int threads, cudaStream_t st, int32_t* bins,
                        double* x, double* jac, double* f, double* wf, int32_t* pass)
@@ -137,8 +151,19 @@ cudaError_t inst_occupancy(const Instance* in, int* ctas, int threads, size_t sm
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t launch_iterate(const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB><<<grid, threads, smem, st>>>(a);
-    return cudaGetLastError();
+    // programmatic stream serialization: this launch may begin (its shared-memory prologue, up to griddepcontrol.wait)
+    // while the kernel in front of it on the stream is still in its tail
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid));
+    cfg.blockDim = dim3(static_cast<unsigned>(threads));
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB>, a);
 }
 template <class F, int D>
 cudaError_t launch_debug(const IterArgs& a, int grid, int threads, cudaStream_t st, int32_t* bins, double* x,
@@ -264,6 +289,7 @@ struct vegas_ctx {
     int n_user_params;
     int use_graph;                   // vegas_run_integration replays a captured step (vegas_use_cuda_graph)
     cudaGraphExec_t gexec;           // captured {memset, launches, finalize, refine, commit} for the key below
+    cudaGraphExec_t gexec_k;         // kStepsPerGraph of them in one graph (single-launch steps only)
     uint64_t g_n, g_epl, g_seed; double g_alpha; int g_threads, g_ctas, g_rshift; const Instance* g_inst;
     cudaStream_t lane[kLanes];       // non-blocking streams: small launches of one iteration overlap on the GPU
     cudaEvent_t lane_done[kLanes], fork;
@@ -508,7 +534,7 @@ static int create_common(vegas_ctx** out, int dim, int nbins, int integrand_id, 
     c->ws = static_cast<unsigned char*>(dev_workspace);
     c->L = L;
     c->iteration = 0; c->have_hist = false; c->have_sums = false;
-    c->h_result = nullptr; c->h_status = nullptr; c->h_ring = nullptr; c->run_ev0 = nullptr; c->run_ev1 = nullptr; c->gstream = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0; c->use_graph = 1; c->gexec = nullptr;
+    c->h_result = nullptr; c->h_status = nullptr; c->h_ring = nullptr; c->run_ev0 = nullptr; c->run_ev1 = nullptr; c->gstream = nullptr; c->fork = nullptr; c->n_enqueued = 0; c->refine_pending = 0; c->use_graph = 1; c->gexec = nullptr; c->gexec_k = nullptr;
     for (int i = 0; i < kEvPool; ++i) { c->evA[i] = nullptr; c->evB[i] = nullptr; }
     for (int i = 0; i < kLanes; ++i) { c->lane[i] = nullptr; c->lane_done[i] = nullptr; }
     c->last_n = 0; c->last_launches = 0; c->rt_lib = nullptr; c->rt_inst = nullptr;
@@ -600,6 +626,7 @@ void vegas_destroy(vegas_ctx* c)
         if (c->evB[i]) cudaEventDestroy(c->evB[i]);
     }
     if (c->gexec) cudaGraphExecDestroy(c->gexec);
+    if (c->gexec_k) cudaGraphExecDestroy(c->gexec_k);
     if (c->igexec) cudaGraphExecDestroy(c->igexec);
     if (c->rt_lib) cudaLibraryUnload(c->rt_lib);
     delete c->rt_inst;
@@ -1130,33 +1157,52 @@ int vegas_combine_iterations(int n, const double* I, const double* sg, double* m
     return VEGAS_OK;
 }
 
+static void drop_step_graphs(vegas_ctx* c)
+{
+    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
+    if (c->gexec_k) { cudaGraphExecDestroy(c->gexec_k); c->gexec_k = nullptr; }
+}
+
 // Capture one whole step {memset, iterate launches, finalize, refine, commit} of (n_events, epl, seed, alpha) with
 // the current launch shape into a CUDA graph (kept until the key changes).  In the captured step the iteration
 // counter lives in device memory: finalize logs (I, sigma) to a ring and advances it.
-static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha)
+static int capture_steps(vegas_ctx* c, int steps, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha, cudaGraphExec_t* out)
 {
-    if (c->gexec && c->g_n == n_events && c->g_epl == epl && c->g_seed == seed && c->g_alpha == alpha &&
-        c->g_threads == c->threads && c->g_ctas == c->ctas_per_sm && c->g_rshift == c->rshift && c->g_inst == c->inst)
-        return VEGAS_OK;
-    if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }
     CUDA_TRY(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeRelaxed));
     // one kernel per launch, the last CTA of the iteration refines (fused step); two kernels if the launch shape has too
     // little shared memory for that.  No memset either way: run_steps_graph_on clears the accumulators once before the
     // first replay and every step leaves them clean.
-    int rc;
-    if (can_fuse_refine(c)) rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false, alpha);
-    else {
-        rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false);     // (carries its memset)
-        if (rc == VEGAS_OK) { c->have_hist = true; rc = vegas_refine_enqueue(c, alpha); }
+    int rc = VEGAS_OK;
+    for (int k = 0; k < steps && rc == VEGAS_OK; ++k) {
+        if (can_fuse_refine(c)) rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false, alpha);
+        else {
+            rc = enqueue_iteration(c, n_events, 0, n_events, epl, seed, nullptr, kGraphStep, false);     // (carries its memset)
+            if (rc == VEGAS_OK) { c->have_hist = true; rc = vegas_refine_enqueue(c, alpha); }
+        }
     }
     cudaGraph_t graph = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->stream, &graph);     // always leave capture mode
     c->refine_pending = 0;
     if (rc != VEGAS_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
     if (e != cudaSuccess) return fail(VEGAS_ECUDA, "cudaStreamEndCapture failed: %s", cudaGetErrorString(e));
-    const cudaError_t e2 = cudaGraphInstantiate(&c->gexec, graph, 0);
+    const cudaError_t e2 = cudaGraphInstantiate(out, graph, 0);
     cudaGraphDestroy(graph);
-    if (e2 != cudaSuccess) { c->gexec = nullptr; return fail(VEGAS_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    if (e2 != cudaSuccess) { *out = nullptr; return fail(VEGAS_ECUDA, "cudaGraphInstantiate failed: %s", cudaGetErrorString(e2)); }
+    return VEGAS_OK;
+}
+
+// Two graphs per key: one step, and kStepsPerGraph consecutive steps (a graph launch costs ~1 us between two steps, and
+// inside one graph the kernels of consecutive single-launch steps are linked by programmatic dependent launch).
+static int ensure_step_graph(vegas_ctx* c, uint64_t n_events, uint64_t epl, uint64_t seed, double alpha)
+{
+    if (c->gexec && c->g_n == n_events && c->g_epl == epl && c->g_seed == seed && c->g_alpha == alpha &&
+        c->g_threads == c->threads && c->g_ctas == c->ctas_per_sm && c->g_rshift == c->rshift && c->g_inst == c->inst)
+        return VEGAS_OK;
+    drop_step_graphs(c);
+    int rc = capture_steps(c, 1, n_events, epl, seed, alpha, &c->gexec);
+    // many-launch steps are long enough for the graph boundary not to matter (and their graphs are large)
+    if (rc == VEGAS_OK && (n_events + epl - 1) / epl == 1) rc = capture_steps(c, kStepsPerGraph, n_events, epl, seed, alpha, &c->gexec_k);
+    if (rc != VEGAS_OK) { drop_step_graphs(c); return rc; }
     c->g_n = n_events; c->g_epl = epl; c->g_seed = seed; c->g_alpha = alpha;
     c->g_threads = c->threads; c->g_ctas = c->ctas_per_sm; c->g_rshift = c->rshift; c->g_inst = c->inst;
     return VEGAS_OK;
@@ -1201,7 +1247,10 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     long long t_prev = 0;
     for (int done = 0; done < total;) {
         const int chunk = (total - done < kRing) ? total - done : kRing;
-        for (int i = 0; i < chunk; ++i) CUDA_TRY(cudaGraphLaunch(c->gexec, c->stream));
+        for (int i = 0; i < chunk;) {
+            if (c->gexec_k && chunk - i >= kStepsPerGraph) { CUDA_TRY(cudaGraphLaunch(c->gexec_k, c->stream)); i += kStepsPerGraph; }
+            else { CUDA_TRY(cudaGraphLaunch(c->gexec, c->stream)); i += 1; }
+        }
         if (done + chunk == total) CUDA_TRY(cudaEventRecord(c->run_ev1, c->stream));
         CUDA_TRY(cudaMemcpyAsync(c->h_ring, ring, (kRing * 3 + 1) * 8, cudaMemcpyDeviceToHost, c->stream));
         CUDA_TRY(cudaStreamSynchronize(c->stream));
@@ -1242,6 +1291,7 @@ int vegas_set_table(vegas_ctx* c, const double* values, int n)
     c->ic.tab = reinterpret_cast<const double*>(c->ws + c->L.idata);
     c->ic.ntab = n;
     if (c->gexec) { cudaGraphExecDestroy(c->gexec); c->gexec = nullptr; }   // captured kernel arguments are stale
+    if (c->gexec_k) { cudaGraphExecDestroy(c->gexec_k); c->gexec_k = nullptr; }
     if (c->igexec) { cudaGraphExecDestroy(c->igexec); c->igexec = nullptr; }
     return VEGAS_OK;
 }

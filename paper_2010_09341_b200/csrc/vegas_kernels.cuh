@@ -277,8 +277,15 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
 
     const int tid = threadIdx.x;
     const int lane = tid & 31;
-    const uint32_t it = a.iter_ptr ? *a.iter_ptr : a.iteration;   // S1 counter word 2
+    // Programmatic dependent launch: the launch that follows this one on the stream may start now and run its own
+    // prologue up to its griddepcontrol.wait, which returns once this whole grid has completed and its writes are
+    // visible.  Everything before the wait touches shared memory only; the table (rewritten by the previous step's
+    // refinement), the iteration counter, the slots and H are read or written after it.  Without the launch attribute
+    // (or with no kernel in front) both instructions do nothing.
+    asm volatile("griddepcontrol.launch_dependents;");
     for (int i = tid; i < cells * R; i += blockDim.x) sh_hist[i] = 0.0;
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint32_t it = a.iter_ptr ? *a.iter_ptr : a.iteration;   // S1 counter word 2
     {
         const real2* gt = static_cast<const real2*>(a.table);
         for (int i = tid; i < cells * TREP; i += blockDim.x) sh_tab[i] = gt[i / TREP];

@@ -98,6 +98,27 @@ def test_run_integration_parity(name, n, epl, warm):
 
 
 @pytest.mark.gpu
+def test_run_integration_parity_across_a_multi_step_graph():
+    """20 iterations of cfg1 (1e5 events, one launch each): run_integration replays one CUDA graph of 16 consecutive
+    steps -- their kernels linked by programmatic dependent launch -- and four single-step graphs; every iteration is
+    compared with the oracle's free-running driver."""
+    import torch
+    assert torch.cuda.is_available()
+    from oracle import oracle as O
+    from paper_2010_09341_b200 import vegas as V
+    w = W.cfg1()
+    g = V.from_workload(w)
+    o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    gm, ge, gc, info = g.run_integration(18, w.n_events, 0, w.seed, w.alpha, n_warmup=2)
+    om, oe, oc, oI, os_ = o.run_integration(18, w.n_events, w.seed, w.alpha, n_warmup=2, threads=8)
+    np.testing.assert_allclose(info["integral"], oI, rtol=1e-10)
+    np.testing.assert_allclose(info["error"], os_, rtol=1e-10)
+    assert gm == pytest.approx(om, rel=1e-10) and ge == pytest.approx(oe, rel=1e-10)
+    assert g.iteration == o.iteration == 20 and np.all(info["kernel_ms"] > 0)
+    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-10
+
+
+@pytest.mark.gpu
 def test_run_integration_graph_many_iterations_and_speed():
     """More iterations than the device-side result ring holds (64), and the graph replay is not slower than
     the loop of blocking calls on the latency-bound configuration (cfg1)."""
