@@ -113,21 +113,30 @@ struct Instance {
 // VEGAS_NO_PDL=1 in the environment switches programmatic dependent launch off (plain stream order)
 const bool g_use_pdl = [] { const char* e = std::getenv("VEGAS_NO_PDL"); return !(e && e[0] == '1'); }();
 
-// One interface for compiled-in and run-time compiled instances.
-cudaError_t inst_launch(const Instance* in, const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+// Launch configuration of every iterate_kernel launch: programmatic stream serialization allowed, i.e. the launch may
+// begin (its shared-memory prologue, up to griddepcontrol.wait) while the kernel in front of it on the stream is still
+// in its tail.  `attr` must outlive the returned configuration.
+cudaLaunchConfig_t iterate_launch_config(int grid, int threads, size_t smem, cudaStream_t st, cudaLaunchAttribute* attr)
 {
-    if (!in->rt_iterate) return in->launch(a, grid, threads, smem, st);
-    void* args[] = {const_cast<IterArgs*>(&a)};
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid));
     cfg.blockDim = dim3(static_cast<unsigned>(threads));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = g_use_pdl ? 1 : 0;
+    return cfg;
+}
+
+// One interface for compiled-in and run-time compiled instances.
+cudaError_t inst_launch(const Instance* in, const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
+{
+    if (!in->rt_iterate) return in->launch(a, grid, threads, smem, st);
+    void* args[] = {const_cast<IterArgs*>(&a)};
+    cudaLaunchAttribute attr[1];
+    const cudaLaunchConfig_t cfg = iterate_launch_config(grid, threads, smem, st, attr);
     return cudaLaunchKernelExC(&cfg, in->rt_iterate, args);
 }
 cudaError_t inst_debug(const Instance* in, const IterArgs& a, int grid, int threads, cudaStream_t st, int32_t* bins,
@@ -151,18 +160,8 @@ cudaError_t inst_occupancy(const Instance* in, int* ctas, int threads, size_t sm
 template <class F, int D, int NB, int RS, int TREP, int HB, int MAXT, int MINB>
 cudaError_t launch_iterate(const IterArgs& a, int grid, int threads, size_t smem, cudaStream_t st)
 {
-    // programmatic stream serialization: this launch may begin (its shared-memory prologue, up to griddepcontrol.wait)
-    // while the kernel in front of it on the stream is still in its tail
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(static_cast<unsigned>(grid));
-    cfg.blockDim = dim3(static_cast<unsigned>(threads));
-    cfg.dynamicSmemBytes = smem;
-    cfg.stream = st;
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    const cudaLaunchConfig_t cfg = iterate_launch_config(grid, threads, smem, st, attr);
     return cudaLaunchKernelEx(&cfg, iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB>, a);
 }
 template <class F, int D>
