@@ -243,13 +243,16 @@ __device__ __forceinline__ void cta_tail(const IterArgs& a, Comp s1, Comp s2, un
     __syncthreads();
     if (!sh_last) return;
     __threadfence();                                     // see the other CTAs' slots and histogram reductions
-    if (tid < 32)
+    // S6 by one warp.  In a fused step it is the CTA's last warp, which has the least to do in the first steps of S7
+    // (no bins of its own to load), so that S6 runs beside them; S7's block barriers then order S6's reads of the slots
+    // and the pass counter before they are cleared below.
+    const bool fused = a.refine_alpha >= 0.0;
+    if (warp == (fused ? nwarps - 1 : 0))
         finalize_warp(a.slots0, a.fin_lanes, a.fin_stride, a.fin_used, a.npass, a.n_events, a.partials, a.result,
                       a.dev_iter, a.ring, a.ring_len);
-    if (a.refine_alpha >= 0.0) {
+    if (fused) {
         // ---- fused step: S7 by the same CTA, in the shared memory the event loop no longer needs; then the
         // accumulators are cleared, so the next step needs no memset ----
-        __syncthreads();                                 // S6 has read the slots and the pass counter
         refine_all(a.edges, a.hist, N, a.refine_alpha, a.new_edges, d, const_cast<void*>(a.table), a.precision, a.status,
                    smem_raw, static_cast<size_t>(a.smem_bytes), true);
         for (int i = tid; i < a.fin_lanes * a.fin_used * 4; i += blockDim.x) a.slots0[i] = 0.0;
@@ -605,8 +608,7 @@ __device__ __forceinline__ void refine_all(double* edges, double* hist, int N, d
     if (group > kMaxDim) group = kMaxDim;
     const int chunk = (N + 31) >> 5;
     const int lo = lane * chunk < N ? lane * chunk : N, hi = (lo + chunk < N) ? lo + chunk : N;
-    if (tid == 0) sh_bad = 0;
-    __syncthreads();
+    if (tid == 0) sh_bad = 0;                            // first set after several block barriers (step 7 check)
     for (int k0 = 0; k0 < d; k0 += group) {
         const int nd = (d - k0 < group) ? d - k0 : group;
         const int wpd = nwarps / nd;                     // warps per dimension in the element-wise steps (>= 1)
