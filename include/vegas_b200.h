@@ -283,6 +283,19 @@ int vegas_combine_iterations(int n, const double* integral, const double* error,
 int vegas_tune_events_per_launch(vegas_ctx* ctx, uint64_t n_events, uint64_t seed, const uint64_t* candidates,
                                  int n_candidates, uint64_t* best, double* ms);
 
+/* The launch geometry vegas_iterate uses when an iteration is cut into several launches (BASELINE.json configs[2], the
+ * batch-size study of PAPER.md:L57-L65): the launches are dealt to `stream_lanes` internal streams
+ * (min(launches, 128): the kernels a device runs concurrently) and each gets `ctas_per_launch` CTAs, the g that
+ * minimises  ceil(L g / min(cta_slots, lanes g)) x (3 + events_per_launch / (g threads_per_cta))  -- the number of waves
+ * the L launches' CTAs run in, times the length of a CTA in events per thread (3 = its fixed cost: zeroing and flushing
+ * the shared histogram, staging the table, the launch).  One launch: all `cta_slots` CTAs (fewer only if there are not
+ * 32 events for each).  Pure host arithmetic: no device, no context.  `cta_slots` = CTAs resident on the device
+ * (vegas_device_info: sm_count x ctas_per_sm of the launch shape).  Any output pointer may be NULL.
+ * Errors: VEGAS_EINVAL (a zero argument, threads_per_cta outside 32..1024, cta_slots outside 1..2048, more than 2^20
+ * launches). */
+int vegas_plan_launches(uint64_t n_events, uint64_t events_per_launch, int threads_per_cta, int cta_slots, int* n_launches,
+                        int* stream_lanes, int* ctas_per_launch);
+
 /* Measured instruction throughput (thread-instructions per second over the whole GPU, current clocks) of
  * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports
  * (BASELINE.json north_star: "fraction of the FP pipe roofline").  Each call runs a

@@ -682,6 +682,31 @@ enum IterMode {
                        // host before every replay
 };
 
+// The wave model behind the launch geometry (see enqueue_iteration): stream lanes and CTAs per launch for `count`
+// events cut into launches of `epl`, with `threads` per CTA and `cta_slots` CTAs resident on the device.  Pure host
+// arithmetic (exported as vegas_plan_launches for the tests and the report).
+static void plan_launches(uint64_t count, uint64_t epl, int threads, int cta_slots, int* lanes_out, int* grid_out)
+{
+    int lanes = 1, grid = cta_slots;
+    const uint64_t n_launches = (count + epl - 1) / epl;
+    if (n_launches > 1) {
+        const double L = static_cast<double>(n_launches);
+        const int lanes_max = n_launches < static_cast<uint64_t>(kLanes) ? static_cast<int>(n_launches) : kLanes;
+        const double per_thread = static_cast<double>(epl < count ? epl : count) / static_cast<double>(threads);
+        double best = 0.0;
+        for (int g = 1; g <= cta_slots; ++g) {
+            const double conc = std::fmin(static_cast<double>(cta_slots), static_cast<double>(lanes_max) * g);
+            const double waves = std::ceil(L * g / conc);
+            const double cost = waves * (kCtaOverheadEvents + per_thread / g);
+            if (g == 1 || cost < best * (1.0 - 1e-9)) { best = cost; grid = g; }
+        }
+        lanes = lanes_max;
+        while (lanes > 1 && static_cast<size_t>(lanes) * grid > static_cast<size_t>(kMaxSlots)) --lanes;
+    }
+    *lanes_out = lanes;
+    *grid_out = grid;
+}
+
 static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
                              uint64_t seed, int* n_kernel_launches, IterMode mode, bool shard, double fuse_alpha = -1.0);
 static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
@@ -844,20 +869,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     // cnt / (g threads) events per thread.  Small g amortises the fixed cost, large g evens out the last wave; the model
     // reproduces the measured times of the batch-size sweep to a few percent.
     int lanes = 1, cap_grid = max_grid;
-    if (n_launches > 1) {
-        const double L = static_cast<double>(n_launches);
-        const int lanes_max = n_launches < static_cast<uint64_t>(kLanes) ? static_cast<int>(n_launches) : kLanes;
-        const double per_thread = static_cast<double>(epl < count ? epl : count) / static_cast<double>(c->threads);
-        double best = 0.0;
-        for (int g = 1; g <= max_grid; ++g) {
-            const double conc = std::fmin(static_cast<double>(max_grid), static_cast<double>(lanes_max) * g);
-            const double waves = std::ceil(L * g / conc);
-            const double cost = waves * (kCtaOverheadEvents + per_thread / g);
-            if (g == 1 || cost < best * (1.0 - 1e-9)) { best = cost; cap_grid = g; }
-        }
-        lanes = lanes_max;
-        while (lanes > 1 && static_cast<size_t>(lanes) * cap_grid > static_cast<size_t>(kMaxSlots)) --lanes;
-    }
+    plan_launches(count, epl, c->threads, max_grid, &lanes, &cap_grid);
     if (lanes > 1) {
         CUDA_TRY(cudaEventRecord(c->fork, c->stream));
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
@@ -924,6 +936,22 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     }
     CUDA_TRY(cudaGetLastError());
     if (n_kernel_launches) *n_kernel_launches = launches;
+    return VEGAS_OK;
+}
+
+int vegas_plan_launches(uint64_t n_events, uint64_t events_per_launch, int threads_per_cta, int cta_slots, int* n_launches,
+                        int* stream_lanes, int* ctas_per_launch)
+{
+    if (n_events < 1 || events_per_launch < 1 || threads_per_cta < 32 || threads_per_cta > 1024 || cta_slots < 1 || cta_slots > kLaneSlots)
+        return fail(VEGAS_EINVAL, "vegas_plan_launches: n_events, events_per_launch >= 1, 32 <= threads_per_cta <= 1024, 1 <= cta_slots <= %d required", kLaneSlots);
+    const uint64_t epl = events_per_launch < n_events ? events_per_launch : n_events;
+    const uint64_t nl = (n_events + epl - 1) / epl;
+    if (nl > kMaxLaunches) return fail(VEGAS_EINVAL, "too many launches for one iteration (raise events_per_launch)");
+    int lanes = 1, grid = cta_slots;
+    plan_launches(n_events, epl, threads_per_cta, cta_slots, &lanes, &grid);
+    if (n_launches) *n_launches = static_cast<int>(nl);
+    if (stream_lanes) *stream_lanes = lanes;
+    if (ctas_per_launch) *ctas_per_launch = grid;
     return VEGAS_OK;
 }
 
