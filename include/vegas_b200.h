@@ -289,12 +289,14 @@ int vegas_tune_events_per_launch(vegas_ctx* ctx, uint64_t n_events, uint64_t see
  * minimises  ceil(L g / min(cta_slots, lanes g)) x (3 + events_per_launch / (g threads_per_cta))  -- the number of waves
  * the L launches' CTAs run in, times the length of a CTA in events per thread (3 = its fixed cost: zeroing and flushing
  * the shared histogram, staging the table, the launch).  One launch: all `cta_slots` CTAs (fewer only if there are not
- * 32 events for each).  Pure host arithmetic: no device, no context.  `cta_slots` = CTAs resident on the device
+ * 32 events for each).  When lanes x g CTAs do not cover the CTA slots (the device runs at most 128 kernels at a time:
+ * launches of one CTA each on 148 SMs) every `extra_cta_every`-th launch gets one CTA more (0: none), aiming at 1.15 x
+ * the slots in flight.  Pure host arithmetic: no device, no context.  `cta_slots` = CTAs resident on the device
  * (vegas_device_info: sm_count x ctas_per_sm of the launch shape).  Any output pointer may be NULL.
  * Errors: VEGAS_EINVAL (a zero argument, threads_per_cta outside 32..1024, cta_slots outside 1..2048, more than 2^20
  * launches). */
 int vegas_plan_launches(uint64_t n_events, uint64_t events_per_launch, int threads_per_cta, int cta_slots, int* n_launches,
-                        int* stream_lanes, int* ctas_per_launch);
+                        int* stream_lanes, int* ctas_per_launch, int* extra_cta_every);
 
 /* Measured instruction throughput (thread-instructions per second over the whole GPU, current clocks) of
  * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports

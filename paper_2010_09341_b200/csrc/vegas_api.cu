@@ -29,6 +29,7 @@ constexpr int kLanes = 128;             // internal streams the launches of one 
                                         // device runs kernels concurrently
 constexpr double kCtaOverheadEvents = 3.0;   // a CTA's prologue + flush + launch cost, in events per thread (measured on
                                         // configs[1]: ~6 us against 2.2 us per event and thread of a full SM)
+constexpr double kOversubscribe = 1.15;  // CTAs in flight aimed at, relative to the CTA slots, when launches are tiny (plan_launches)
 constexpr int kLaneSlots = 2048;        // upper bound on the iterate grid (CTAs) = slots of a lane's region
 constexpr int kMaxSlots = 8 * kLaneSlots;   // lanes x (largest grid among the launches) never exceeds this
 constexpr size_t kStaticSmemReserve = 1024;   // the opt-in shared-memory limit covers static + dynamic: room for the kernels' few static words
@@ -685,9 +686,9 @@ enum IterMode {
 // The wave model behind the launch geometry (see enqueue_iteration): stream lanes and CTAs per launch for `count`
 // events cut into launches of `epl`, with `threads` per CTA and `cta_slots` CTAs resident on the device.  Pure host
 // arithmetic (exported as vegas_plan_launches for the tests and the report).
-static void plan_launches(uint64_t count, uint64_t epl, int threads, int cta_slots, int* lanes_out, int* grid_out)
+static void plan_launches(uint64_t count, uint64_t epl, int threads, int cta_slots, int* lanes_out, int* grid_out, int* extra_every_out)
 {
-    int lanes = 1, grid = cta_slots;
+    int lanes = 1, grid = cta_slots, extra_every = 0;
     const uint64_t n_launches = (count + epl - 1) / epl;
     if (n_launches > 1) {
         const double L = static_cast<double>(n_launches);
@@ -702,9 +703,18 @@ static void plan_launches(uint64_t count, uint64_t epl, int threads, int cta_slo
         }
         lanes = lanes_max;
         while (lanes > 1 && static_cast<size_t>(lanes) * grid > static_cast<size_t>(kMaxSlots)) --lanes;
+        // The device runs at most kLanes kernels at a time: when lanes x grid CTAs do not cover its CTA slots (tiny
+        // launches: 128 one-CTA kernels on 148 SMs) every `extra_every`-th launch gets one CTA more, aiming at 1.15 x the
+        // slots in flight (measured on configs[2] at 1e4 events per launch: 2.90 ms per 1e8 events with none, 2.77 with
+        // every 6th -- exactly the slots --, 2.67 with every 3rd, 2.77 / 2.81 with every 2nd / every one).
+        if (lanes * grid < cta_slots) {
+            const double f = kOversubscribe * static_cast<double>(cta_slots) / (static_cast<double>(lanes) * grid) - 1.0;
+            if (f > 0.02) extra_every = f >= 1.0 ? 1 : static_cast<int>(1.0 / f + 0.5);
+        }
     }
     *lanes_out = lanes;
     *grid_out = grid;
+    *extra_every_out = extra_every;
 }
 
 static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64_t count, uint64_t events_per_launch,
@@ -868,8 +878,8 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     // the shared histogram, staging the table, the launch itself: kCtaOverheadEvents events per thread) plus
     // cnt / (g threads) events per thread.  Small g amortises the fixed cost, large g evens out the last wave; the model
     // reproduces the measured times of the batch-size sweep to a few percent.
-    int lanes = 1, cap_grid = max_grid;
-    plan_launches(count, epl, c->threads, max_grid, &lanes, &cap_grid);
+    int lanes = 1, cap_grid = max_grid, extra_every = 0;
+    plan_launches(count, epl, c->threads, max_grid, &lanes, &cap_grid, &extra_every);
     if (lanes > 1) {
         CUDA_TRY(cudaEventRecord(c->fork, c->stream));
         for (int i = 0; i < lanes; ++i) CUDA_TRY(cudaStreamWaitEvent(c->lane[i], c->fork, 0));
@@ -884,22 +894,26 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
         const uint64_t to_wrap = (uint64_t(1) << 32) - (at & 0xFFFFFFFFull);    // never straddle 2^32 (e_hi uniform)
         return cnt > to_wrap ? to_wrap : cnt;
     };
-    auto launch_grid = [&](uint64_t cnt) {
+    auto launch_grid = [&](uint64_t cnt, int index) {
         // one launch: spread even few events over all SMs (the CTAs' fixed costs run side by side; at least a warp of
         // events each); several launches share the GPU: never more threads than events
         const uint64_t per_cta = (n_launches == 1) ? 32u : static_cast<uint64_t>(c->threads);
         uint64_t want = (cnt + per_cta - 1) / per_cta;
         if (want < 1) want = 1;
-        return want < static_cast<uint64_t>(cap_grid) ? static_cast<int>(want) : cap_grid;
+        const int cap = cap_grid + ((extra_every > 0 && index % extra_every == 0) ? 1 : 0);
+        return want < static_cast<uint64_t>(cap) ? static_cast<int>(want) : cap;
     };
     uint64_t total_ctas = 0;
     int used_grid = 0;
-    for (uint64_t at = first; at < last;) {
-        const uint64_t cnt = launch_count(at);
-        const int grid = launch_grid(cnt);
-        total_ctas += static_cast<uint64_t>(grid);
-        if (grid > used_grid) used_grid = grid;
-        at += cnt;
+    {
+        int index = 0;
+        for (uint64_t at = first; at < last; ++index) {
+            const uint64_t cnt = launch_count(at);
+            const int grid = launch_grid(cnt, index);
+            total_ctas += static_cast<uint64_t>(grid);
+            if (grid > used_grid) used_grid = grid;
+            at += cnt;
+        }
     }
     if (total_ctas > 0xFFFFFFFFull) return fail(VEGAS_EINVAL, "too many launches for one iteration (raise events_per_launch)");
     a.ticket = reinterpret_cast<unsigned int*>(c->ws + c->L.npass) + 4;   // inside the region cleared by the memset
@@ -921,7 +935,7 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
         a.e_lo_first = static_cast<uint32_t>(at);
         a.e_hi = static_cast<uint32_t>(at >> 32);
         a.count = static_cast<uint32_t>(cnt);
-        const int grid = launch_grid(cnt);
+        const int grid = launch_grid(cnt, launches);
         const int ln = launches % lanes;
         a.slots = slots0 + static_cast<size_t>(ln) * used_grid * 4;
         CUDA_TRY(inst_launch(c->inst, a, grid, c->threads, c->smem_bytes, lanes > 1 ? c->lane[ln] : c->stream));
@@ -940,18 +954,19 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
 }
 
 int vegas_plan_launches(uint64_t n_events, uint64_t events_per_launch, int threads_per_cta, int cta_slots, int* n_launches,
-                        int* stream_lanes, int* ctas_per_launch)
+                        int* stream_lanes, int* ctas_per_launch, int* extra_cta_every)
 {
     if (n_events < 1 || events_per_launch < 1 || threads_per_cta < 32 || threads_per_cta > 1024 || cta_slots < 1 || cta_slots > kLaneSlots)
         return fail(VEGAS_EINVAL, "vegas_plan_launches: n_events, events_per_launch >= 1, 32 <= threads_per_cta <= 1024, 1 <= cta_slots <= %d required", kLaneSlots);
     const uint64_t epl = events_per_launch < n_events ? events_per_launch : n_events;
     const uint64_t nl = (n_events + epl - 1) / epl;
     if (nl > kMaxLaunches) return fail(VEGAS_EINVAL, "too many launches for one iteration (raise events_per_launch)");
-    int lanes = 1, grid = cta_slots;
-    plan_launches(n_events, epl, threads_per_cta, cta_slots, &lanes, &grid);
+    int lanes = 1, grid = cta_slots, extra = 0;
+    plan_launches(n_events, epl, threads_per_cta, cta_slots, &lanes, &grid, &extra);
     if (n_launches) *n_launches = static_cast<int>(nl);
     if (stream_lanes) *stream_lanes = lanes;
     if (ctas_per_launch) *ctas_per_launch = grid;
+    if (extra_cta_every) *extra_cta_every = extra;
     return VEGAS_OK;
 }
 

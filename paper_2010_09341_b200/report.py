@@ -49,7 +49,7 @@ def run_config(name, w, n_iter=None, epl=0, tune=False):
            "events_per_s_median": w.n_events / (statistics.median(ms) * 1e-3),
            "events_per_s_best": w.n_events / (min(ms) * 1e-3),
            "wall_ms_median": statistics.median(wall), "refine_ms_median": statistics.median(rms), "launch_shape": g.launch_shape(),
-           "launch_plan": dict(zip(("launches", "stream_lanes", "ctas_per_launch"),
+           "launch_plan": dict(zip(("launches", "stream_lanes", "ctas_per_launch", "extra_cta_every"),
                                    V.plan_launches(w.n_events, epl or w.n_events, g.launch_shape()["threads_per_cta"],
                                                    g.device_info()["sm_count"] * g.launch_shape()["ctas_per_sm"]))),
            "pass_fraction_first_last": [passf[0], passf[-1]], "last_result": res[-1],

@@ -55,7 +55,7 @@ SIGNATURES = {
                                         _dp, _dp, _dp, _dp]),
     "vegas_tune_events_per_launch": (C.c_int, [_vp, C.c_uint64, C.c_uint64, _u64p, C.c_int, _u64p, _dp]),
     "vegas_use_cuda_graph": (C.c_int, [_vp, C.c_int]),
-    "vegas_plan_launches": (C.c_int, [C.c_uint64, C.c_uint64, C.c_int, C.c_int, _ip, _ip, _ip]),
+    "vegas_plan_launches": (C.c_int, [C.c_uint64, C.c_uint64, C.c_int, C.c_int, _ip, _ip, _ip, _ip]),
     "vegas_combine_iterations": (C.c_int, [C.c_int, _dp, _dp, _dp, _dp, _dp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
@@ -97,12 +97,12 @@ def workspace_bytes(dim, nbins):
 
 
 def plan_launches(n_events, events_per_launch, threads_per_cta, cta_slots):
-    """(launches, stream lanes, CTAs per launch) of an iteration cut into launches: the library's wave model
-    (vegas_plan_launches; host arithmetic only)."""
-    nl, lanes, grid = C.c_int(), C.c_int(), C.c_int()
+    """(launches, stream lanes, CTAs per launch, every how many launches one CTA more) of an iteration cut into
+    launches: the library's wave model (vegas_plan_launches; host arithmetic only)."""
+    nl, lanes, grid, extra = C.c_int(), C.c_int(), C.c_int(), C.c_int()
     _chk(lib().vegas_plan_launches(int(n_events), int(events_per_launch), int(threads_per_cta), int(cta_slots),
-                                   C.byref(nl), C.byref(lanes), C.byref(grid)), "vegas_plan_launches")
-    return nl.value, lanes.value, grid.value
+                                   C.byref(nl), C.byref(lanes), C.byref(grid), C.byref(extra)), "vegas_plan_launches")
+    return nl.value, lanes.value, grid.value, extra.value
 
 
 class Vegas:

@@ -114,28 +114,29 @@ def test_plan_launches_wave_model():
     for the batch-size sweep of configs[2] on 148 SMs x 768 threads, and the model's invariants."""
     from paper_2010_09341_b200 import vegas
     n = 10**8
-    assert vegas.plan_launches(n, 10**4, 768, 148) == (10000, 128, 1)
-    assert vegas.plan_launches(n, 10**5, 768, 148) == (1000, 128, 2)
-    assert vegas.plan_launches(n, 10**6, 768, 148) == (100, 100, 16)
-    assert vegas.plan_launches(n, 10**7, 768, 148) == (10, 10, 59)
-    assert vegas.plan_launches(n, n, 768, 148) == (1, 1, 148)
-    assert vegas.plan_launches(n, 2 * n, 768, 148) == (1, 1, 148)          # events_per_launch is capped at n_events
+    assert vegas.plan_launches(n, 10**4, 768, 148) == (10000, 128, 1, 3)
+    assert vegas.plan_launches(n, 10**5, 768, 148) == (1000, 128, 2, 0)
+    assert vegas.plan_launches(n, 10**6, 768, 148) == (100, 100, 16, 0)
+    assert vegas.plan_launches(n, 10**7, 768, 148) == (10, 10, 59, 0)
+    assert vegas.plan_launches(n, n, 768, 148) == (1, 1, 148, 0)
+    assert vegas.plan_launches(n, 2 * n, 768, 148) == (1, 1, 148, 0)          # events_per_launch is capped at n_events
     for epl in (1, 7, 999, 12345, 10**6 + 3):
         for threads, slots in ((64, 148), (1024, 296), (256, 2048)):
             m = 10**6 + 3
             if (m + epl - 1) // epl > 2**20:
                 continue
-            nl, lanes, grid = vegas.plan_launches(m, epl, threads, slots)
+            nl, lanes, grid, extra = vegas.plan_launches(m, epl, threads, slots)
             assert nl == (m + epl - 1) // epl and 1 <= lanes <= min(nl, 128) and 1 <= grid <= slots
-            assert lanes * grid <= 16384                                       # slot regions of the workspace
+            assert extra >= 0 and (extra == 0 or lanes * grid < slots)
+            assert lanes * (grid + 1) <= 16384                                       # slot regions of the workspace
     # the model's cost is never worse than the two extreme grids
     import math
     def cost(L, per_thread, g, slots, lanes): return math.ceil(L * g / min(slots, lanes * g)) * (3.0 + per_thread / g)
-    nl, lanes, grid = vegas.plan_launches(n, 10**6, 768, 148)
+    nl, lanes, grid, _ = vegas.plan_launches(n, 10**6, 768, 148)
     assert cost(nl, 1e6 / 768, grid, 148, lanes) <= min(cost(nl, 1e6 / 768, 1, 148, lanes), cost(nl, 1e6 / 768, 148, 148, lanes))
     L = vegas.lib()
-    assert L.vegas_plan_launches(0, 1, 768, 148, None, None, None) == vegas.EINVAL
-    assert L.vegas_plan_launches(10, 0, 768, 148, None, None, None) == vegas.EINVAL
-    assert L.vegas_plan_launches(10, 1, 16, 148, None, None, None) == vegas.EINVAL
-    assert L.vegas_plan_launches(10**8, 1, 768, 148, None, None, None) == vegas.EINVAL      # 1e8 launches
-    assert L.vegas_plan_launches(10, 5, 768, 148, None, None, None) == vegas.OK
+    assert L.vegas_plan_launches(0, 1, 768, 148, None, None, None, None) == vegas.EINVAL
+    assert L.vegas_plan_launches(10, 0, 768, 148, None, None, None, None) == vegas.EINVAL
+    assert L.vegas_plan_launches(10, 1, 16, 148, None, None, None, None) == vegas.EINVAL
+    assert L.vegas_plan_launches(10**8, 1, 768, 148, None, None, None, None) == vegas.EINVAL      # 1e8 launches
+    assert L.vegas_plan_launches(10, 5, 768, 148, None, None, None, None) == vegas.OK

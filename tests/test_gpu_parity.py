@@ -407,8 +407,8 @@ def test_full_size_cascade(V, O, name):
 def test_cfg3_sweep_parity(V, O):
     """BASELINE.json configs[2]: 1e8 events of the d=8 double Gaussian split into launches of 1e4 ... 1e8 events; every
     split is compared with ONE oracle iteration (not with another GPU run).  The launches are dealt to up to 128 internal
-    streams with the grid the library's wave model picks (10 000 launches of one CTA each, 1 000 of two, 100 of about
-    sixteen, 10 of half the SMs, 1 of all), as a replayed CUDA graph and, for 1e4 / 1e5, also as plain launches."""
+    streams with the grid the library's wave model picks (10 000 launches of one CTA each -- two for every third --, 1 000 of
+    two, 100 of sixteen, 10 of 59, 1 of all), as a replayed CUDA graph and, for 1e4 / 1e5, also as plain launches."""
     w = W.cfg3()
     g, o = make_pair(V, O, w)
     ores = o.iterate(w.n_events, w.seed, threads=THREADS)
