@@ -323,6 +323,47 @@ enum { VEGAS_PIPE_DFMA = 0, VEGAS_PIPE_FFMA = 1, VEGAS_PIPE_IMAD_WIDE = 2, VEGAS
        VEGAS_PIPE_DFMA_3REG = 8, VEGAS_PIPE_MIX_EVENT_LOOP = 9 };
 int vegas_pipe_rate(int pipe, void* cuda_stream, double* thread_instr_per_s);
 
+/* Grid refinement (S7, as vegas_refine computes it) for callers that cannot give the library device memory.
+ *
+ * Every other call works in the workspace the caller allocated for vegas_create.  A caller that runs as a guest in
+ * another program -- a plug-in, a framework callback, a custom operator: it receives device pointers to its inputs and
+ * outputs, while the host program's memory pool already owns almost all of the GPU's memory -- has no allocator to ask:
+ * its own cudaMalloc may fail for lack of free memory, and cudaMalloc / cudaFree hold up the whole device while the
+ * host's streams are busy, which a step inside a pipelined loop must not do.  For them the working memory of the
+ * refinement (candidate edges, a writable copy of the histogram, the rebuilt mapping table, outcome flags) is an array
+ * compiled into the library.  This call needs no context, makes no cudaMalloc / cudaFree and calls no library routine
+ * that allocates.
+ *
+ *   dev_edges     in   device, dim*(nbins+1) doubles, row-major [k][i]: the current grid, 0 = E0 < ... < EN = 1 per row
+ *   dev_hist      in   device, dim*nbins doubles, row-major [k][i]: H of an iteration sampled through that grid
+ *   dev_new_edges out  device, dim*(nbins+1) doubles: the refined grid -- bit-identical to what vegas_refine commits for
+ *                      the same edges, histogram and alpha.  If the refinement is rejected (some dimension's new edges
+ *                      not strictly increasing: vegas_refine's VEGAS_EGRID) it receives a copy of dev_edges.  A
+ *                      dimension whose histogram sums to 0 keeps its edges.  May be the same buffer as dev_edges.
+ *   dev_status    out  device, one int: 0 = refined, 1 = rejected
+ * Inputs and outputs belong to the caller.  The call only enqueues one kernel on `cuda_stream` (NULL = the legacy
+ * default stream) and returns; outputs are valid once the stream reaches that point.  The device that owns the stream
+ * must be the current device.
+ *
+ * Limits and sharing -- read before use:
+ *   - dim * (nbins + 1) <= VEGAS_STATIC_MAX_EDGES (8192; all BASELINE.json configurations are below 2100).  Larger grids
+ *     are refused with VEGAS_EINVAL and a message naming the limit; they need vegas_create + vegas_refine.
+ *   - The array is 4 * VEGAS_STATIC_MAX_EDGES doubles + 256 bytes, about 256 KB, and every GPU on which this library is
+ *     loaded holds it from load until the process exits, whether or not this call is ever made.
+ *   - There is ONE array per device.  Every call uses it, and it keeps the contents of the previous call; the kernel
+ *     resets what has to start from zero (the outcome counters) and overwrites the rest before reading it.  Two calls
+ *     whose kernels can run at the same time on one device (different streams, different host threads) race on it and
+ *     give garbage: serialise them (same stream, or an event between them).
+ *   - The first call on each device does a one-time set-up for that device (it asks the CUDA runtime for the array's
+ *     device address -- cudaGetSymbolAddress -- and raises the kernel's shared-memory limit).  Make that first call
+ *     outside any stream capture, e.g. once at start-up.
+ * Errors: VEGAS_EINVAL (ranges, the size limit, alpha < 0 or NaN, a NULL or misaligned pointer), VEGAS_EUNSUPPORTED (a
+ * device other than sm_100), VEGAS_ECUDA.  Reading: SURVEY 8.c S7; PAPER.md:L88 ("every iteration informs the
+ * subsequent run"). */
+#define VEGAS_STATIC_MAX_EDGES 8192
+int vegas_refine_static_enqueue(int dim, int nbins, double alpha, const double* dev_edges, const double* dev_hist,
+                                double* dev_new_edges, int* dev_status, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

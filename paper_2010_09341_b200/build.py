@@ -15,7 +15,8 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libvegas_b200.so")
-SOURCES = [os.path.join(CSRC, "vegas_api.cu"), os.path.join(CSRC, "pipe_bench.cu"), os.path.join(CSRC, "vegas_rtc.cu")]
+SOURCES = [os.path.join(CSRC, "vegas_api.cu"), os.path.join(CSRC, "pipe_bench.cu"), os.path.join(CSRC, "vegas_rtc.cu"),
+           os.path.join(CSRC, "vegas_static.cu")]
 DEPS = SOURCES + [os.path.join(CSRC, "vegas_kernels.cuh"), os.path.join(CSRC, "vegas_device.cuh"),
                   os.path.join(CSRC, "vegas_user.cuh"), os.path.join(CSRC, "vegas_rtc.h"),
                   os.path.join(INCLUDE, "vegas_b200.h")]

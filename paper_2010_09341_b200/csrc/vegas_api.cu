@@ -261,6 +261,10 @@ int expected_params(int id, int dim)
 
 }  // namespace
 
+// Lets the library's other translation units (vegas_static.cu) record the message vegas_last_error() returns.  Not
+// exported from the shared object.
+__attribute__((visibility("hidden"))) int vegas_detail_fail(int code, const char* msg) { return fail(code, "%s", msg); }
+
 struct vegas_ctx {
     int dim, nbins, integrand_id, precision;
     const Instance* inst;            // the instance in use (tuned or generic, chosen by apply_shape)

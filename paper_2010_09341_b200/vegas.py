@@ -57,6 +57,7 @@ SIGNATURES = {
     "vegas_use_cuda_graph": (C.c_int, [_vp, C.c_int]),
     "vegas_plan_launches": (C.c_int, [C.c_uint64, C.c_uint64, C.c_int, C.c_int, _ip, _ip, _ip, _ip]),
     "vegas_combine_iterations": (C.c_int, [C.c_int, _dp, _dp, _dp, _dp, _dp]),
+    "vegas_refine_static_enqueue": (C.c_int, [C.c_int, C.c_int, C.c_double, _vp, _vp, _vp, _vp, _vp]),
     "vegas_destroy": (None, [_vp]),
     "vegas_last_error": (C.c_char_p, []),
 }
@@ -324,6 +325,26 @@ def pipe_rate(pipe, stream=None):
     _chk(lib().vegas_pipe_rate(int(pipe), _vp(stream.cuda_stream) if stream is not None else None, C.byref(v)),
          "vegas_pipe_rate")
     return v.value
+
+
+STATIC_MAX_EDGES = 8192   # VEGAS_STATIC_MAX_EDGES
+
+
+def _dev_ptr(t):
+    return _vp(int(t.data_ptr()) if hasattr(t, "data_ptr") else int(t))
+
+
+def refine_static_enqueue(dim, nbins, alpha, dev_edges, dev_hist, dev_new_edges, dev_status, stream=None):
+    """vegas_refine_static_enqueue: the refinement for callers that cannot allocate device memory -- guests of
+    another program (plug-ins, framework callbacks) that are handed device buffers while the host's pool owns the
+    rest of the GPU.  No context, no workspace: the working memory is an array compiled into the library (one per
+    device, shared by all calls: do not let two of these calls overlap on a device; dim*(nbins+1) <= STATIC_MAX_EDGES).
+    The buffers are device memory given as torch tensors (float64 edges [dim][nbins+1] and hist [dim][nbins] in,
+    float64 new edges and one int32 status out) or raw addresses.  Enqueues one kernel and returns."""
+    _chk(lib().vegas_refine_static_enqueue(int(dim), int(nbins), float(alpha), _dev_ptr(dev_edges), _dev_ptr(dev_hist),
+                                           _dev_ptr(dev_new_edges), _dev_ptr(dev_status),
+                                           _vp(stream.cuda_stream) if stream is not None else None),
+         "vegas_refine_static_enqueue")
 
 
 def combine_iterations(integral, error):
