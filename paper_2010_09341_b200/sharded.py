@@ -9,7 +9,9 @@ it every rank holds the same sums, runs S6 (vegas_finalize_enqueue) and the iden
 bit-identical on all ranks with no further communication.
 
 `ctx` is anything with the binding's three calls (paper_2010_09341_b200.vegas.Vegas, or a stand-in in the CPU tests):
-iterate_shard_enqueue(n_total, first, count, events_per_launch, seed), partials_tensor(), finalize_enqueue(n_total).
+iterate_shard_enqueue(n_total, first, count, events_per_launch, seed), partials_tensor(), finalize_enqueue(n_total);
+if it has a `stream` attribute (the torch stream its kernels run on) the all-reduce is issued on that stream.
+Never run on more than one device so far (one GPU per box): covered by gloo tests, on CPU and with two ranks on one GPU.
 """
 from __future__ import annotations
 
@@ -40,7 +42,18 @@ def iterate_sharded_enqueue(ctx, n_events: int, events_per_launch: int = 0, seed
     epl = int(events_per_launch) if events_per_launch else max(count, 1)
     launches = ctx.iterate_shard_enqueue(int(n_events), first, count, epl, seed)
     if world > 1:
-        dist.all_reduce(ctx.partials_tensor(), op=dist.ReduceOp.SUM, group=group)   # the iteration's one exchange
+        # The iteration's one exchange.  The collective orders itself against torch's CURRENT stream, while the shard
+        # kernels before it and S6 after it run on the stream the context was created with: make that stream current
+        # for the call, else the sum could read partials the last CTA has not written yet (or S6 read them before the
+        # sum landed) whenever the two streams differ.
+        part = ctx.partials_tensor()
+        stream = getattr(ctx, "stream", None)
+        if stream is not None and part.is_cuda:
+            import torch
+            with torch.cuda.stream(stream):
+                dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
+        else:
+            dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
     ctx.finalize_enqueue(int(n_events))
     return launches
 

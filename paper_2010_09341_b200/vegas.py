@@ -140,6 +140,13 @@ class Vegas:
         self._h = h
         self.dim, self.nbins, self.integrand_id, self.precision = dim, nbins, integrand_id, precision
 
+    @property
+    def stream(self):
+        """The torch stream every kernel of this context runs on (the one given at construction, else the stream that
+        was current then).  Work that reads or writes the context's device memory -- the all-reduce of
+        partials_tensor() -- must be ordered on it."""
+        return self._stream
+
     def close(self):
         if getattr(self, "_h", None):
             lib().vegas_destroy(self._h)

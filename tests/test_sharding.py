@@ -112,6 +112,17 @@ def test_sharded_iteration_equals_unsharded_and_oracle(V, name, G, n, epl):
 
 
 @pytest.mark.gpu
+def test_sharded_iteration_two_ranks_one_gpu_non_default_stream(V):
+    """The real binding under a process group (gloo, two ranks sharing the one GPU), contexts on a non-default stream:
+    the all-reduce must be ordered on the context's stream (tests/_gloo_gpu_shard_worker.py)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", str(_free_port()), os.path.join("tests", "_gloo_gpu_shard_worker.py")]
+    r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    assert "GPU_SHARD_OK world=2" in r.stdout
+
+
+@pytest.mark.gpu
 def test_shard_argument_errors(V):
     w = W.cfg1()
     g = V.from_workload(w)
