@@ -113,6 +113,11 @@ struct Instance {
 
 // VEGAS_NO_PDL=1 in the environment switches programmatic dependent launch off (plain stream order)
 const bool g_use_pdl = [] { const char* e = std::getenv("VEGAS_NO_PDL"); return !(e && e[0] == '1'); }();
+// Cleared by enqueue_iteration around the launches of an iteration that is dealt to several stream lanes: there whole
+// chains of dependent kernels would become resident and sit at griddepcontrol.wait holding shared memory and thread
+// slots that other lanes' kernels need (measured on configs[2], 1e4 events per launch: 2.67 ms with the attribute,
+// 2.62 ms without; 1e5 and up: no difference).  The attribute pays where launches follow one another on ONE stream.
+thread_local bool t_pdl_this_launch = true;
 
 // Launch configuration of every iterate_kernel launch: programmatic stream serialization allowed, i.e. the launch may
 // begin (its shared-memory prologue, up to griddepcontrol.wait) while the kernel in front of it on the stream is still
@@ -127,7 +132,7 @@ cudaLaunchConfig_t iterate_launch_config(int grid, int threads, size_t smem, cud
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = g_use_pdl ? 1 : 0;
+    cfg.numAttrs = (g_use_pdl && t_pdl_this_launch) ? 1 : 0;
     return cfg;
 }
 
@@ -827,6 +832,7 @@ static int iterate_common(vegas_ctx* c, uint64_t n_total, uint64_t first, uint64
         rc = ensure_iter_graph(c, n_total, first, count, events_per_launch, seed, shard, fuse_alpha, &launches);
         if (rc != VEGAS_OK) return rc;
         CUDA_TRY(cudaEventRecord(c->evA[evi], c->stream));
+        c->accum_clean = false;                          // dirty from here on; clean again only if a whole fused step got out
         set_u32_kernel<<<1, 1, 0, c->stream>>>(reinterpret_cast<uint32_t*>(c->ws + c->L.dev_iter), c->iteration);
         CUDA_TRY(cudaGraphLaunch(c->igexec, c->stream));
     } else {
@@ -865,6 +871,10 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     const bool fused = fuse_alpha >= 0.0;
     if (!(fused && (mode == kGraphStep || (mode == kPlain && c->accum_clean))))
         CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    // From the first launch on the accumulators (slots, H, pass counter, ticket) are dirty, and they stay so if a launch
+    // below fails: the last CTA of such a step never runs, so nothing clears them.  iterate_common sets the flag again
+    // once every launch of a fused step was enqueued.  (Captures enqueue nothing: the flag describes the device.)
+    if (mode == kPlain) c->accum_clean = false;
     if (n_kernel_launches) *n_kernel_launches = 0;
     if (count == 0) return VEGAS_OK;                     // an empty shard contributes zeros
     IterArgs a;
@@ -934,6 +944,10 @@ static int enqueue_iteration(vegas_ctx* c, uint64_t n_total, uint64_t first, uin
     a.ring_len = kRing;
     a.refine_alpha = fused ? fuse_alpha : -1.0;
     int launches = 0;
+    struct PdlScope {                                    // programmatic dependent launch only on the single-stream path
+        explicit PdlScope(bool on) { t_pdl_this_launch = on; }
+        ~PdlScope() { t_pdl_this_launch = true; }
+    } pdl_scope(lanes == 1);
     for (uint64_t at = first; at < last;) {
         const uint64_t cnt = launch_count(at);
         a.e_lo_first = static_cast<uint32_t>(at);
@@ -1286,6 +1300,7 @@ static int run_steps_graph_on(vegas_ctx* c, int total, uint64_t n_events, uint64
     CUDA_TRY(cudaMemcpyAsync(c->ws + c->L.dev_iter, h_it, 4, cudaMemcpyHostToDevice, c->stream));
     if (!c->accum_clean)                                 // the captured fused step has no memset of its own
         CUDA_TRY(cudaMemsetAsync(c->ws + c->L.zero_begin, 0, c->L.zero_end - c->L.zero_begin, c->stream));
+    c->accum_clean = false;                              // until every replay below was enqueued and the run was read back
     double* ring = reinterpret_cast<double*>(c->ws + c->L.ring);
     stamp_kernel<<<1, 1, 0, c->stream>>>(ring + 3 * kRing);
     CUDA_TRY(cudaEventRecord(c->run_ev0, c->stream));

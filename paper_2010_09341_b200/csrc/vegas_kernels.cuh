@@ -65,7 +65,7 @@ __device__ __forceinline__ void comp_warp_reduce(Comp& c)
 //   table: TREP lane-indexed copies of every 16-byte (fp64) / 8-byte (fp32) cell, lane l reads copy
 //          l%TREP.  A 16-byte shared load is served one quarter-warp (8 lanes) per wavefront; with TREP = 8
 //          the 8 lanes hit 8 different 4-bank groups whatever their bins are, so the random-bin lookup
-//          costs the minimum 4 wavefronts instead of the ~9.6 measured without replication (profiles/r01a).
+//          costs 3.0 wavefronts per load (profiles/r03_ncu_full_cfg2_iterate.md) instead of the ~9.6 measured in round 1 without replication.
 // Template parameters: D, NB compile-time dimension / bin count (0 = run-time a.dim / a.nbins); RS
 // compile-time log2 R (-1 = run-time a.rshift); TREP; HB = number of histogram updates whose
 // compare-and-swap sequences are issued together (0 = one atomicAdd spin loop per update).
@@ -294,6 +294,10 @@ __global__ void __launch_bounds__(MAXT, MINB) iterate_kernel(const __grid_consta
         for (int i = tid; i < cells * TREP; i += blockDim.x) sh_tab[i] = gt[i / TREP];
     }
     __syncthreads();
+    // lds_cell reads the staged table through plain (non-volatile, no clobber) inline asm, which the compiler sees as a
+    // pure function of the address: this compiler-level fence is what keeps those reads behind the stores above and
+    // the barrier (no instruction is emitted)
+    asm volatile("" ::: "memory");
 
     constexpr int kTCell = TREP * static_cast<int>(sizeof(real2));       // bytes between the table copies of two cells
     constexpr int kHCell = (RS >= 0) ? (8 << (RS >= 0 ? RS : 0)) : 0;    // bytes between two cells' replicas (0: run-time)
@@ -450,7 +454,10 @@ __device__ __forceinline__ void finalize_warp(const double* slots, int nlanes, i
     comp_warp_reduce(t1);
     comp_warp_reduce(t2);
     if (lane == 0) {
-        // renormalise the pairs so that |lo| <= ulp(hi)/2: sums of pairs from several GPUs stay compensated
+        // renormalise the pairs so that |lo| <= ulp(hi)/2.  Across G GPUs the all-reduce adds the hi parts and the lo
+        // parts separately in plain fp64: the lo parts keep each GPU's own compensation, but the G - 1 additions of hi
+        // parts round, so the multi-GPU sum is within (G - 1) ulp/2 of the exact one (1e-15 relative at G = 8), not
+        // compensated like the single-GPU sum
         double h1, l1, h2, l2;
         two_sum(t1.hi, t1.lo, h1, l1);
         two_sum(t2.hi, t2.lo, h2, l2);
