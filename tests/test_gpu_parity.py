@@ -14,6 +14,7 @@ from paper_2010_09341_b200 import workloads as W
 pytestmark = pytest.mark.gpu
 
 THREADS = max(1, min(32, len(os.sched_getaffinity(0))))
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.fixture(scope="module")
@@ -409,6 +410,26 @@ def test_full_size_iteration_parity(V, O, name):
         g.set_grid(o.get_grid())
 
 
+_CASCADE = {}
+
+
+def oracle_cascade(O, name):
+    """The oracle's own free-running full-size run of a configuration -- its n_iter iterations of 1e8 events, a refinement
+    after each -- computed once per test session and shared by the tests that hold different GPU paths against it (the
+    blocking calls, the un-synchronised fused steps bench.py times).  Rows: I, sigma, H, npass, the grid after the refine."""
+    if name not in _CASCADE:
+        w = small_workloads()[name]
+        _, o = None, O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+        rows = []
+        for _ in range(w.n_iter):
+            I, s, h = o.iterate(w.n_events, w.seed, threads=THREADS)
+            npass = o.npass
+            o.refine(w.alpha)
+            rows.append(dict(I=I, s=s, h=h.copy(), npass=npass, grid=o.get_grid().copy()))
+        _CASCADE[name] = rows
+    return _CASCADE[name]
+
+
 @pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
 def test_full_size_cascade(V, O, name):
     """BASELINE.json acceptance at the stated sizes: the configuration's 10 free-running iterations of 1e8 events (the
@@ -417,19 +438,106 @@ def test_full_size_cascade(V, O, name):
     the fifth, which the acceptance names, and all the way to the tenth."""
     w = small_workloads()[name]
     assert w.n_events == 10**8 and w.n_iter == 10
-    g, o = make_pair(V, O, w)
+    rows = oracle_cascade(O, name)
+    g = V.from_workload(w)
     for it in range(w.n_iter):
-        ores = o.iterate(w.n_events, w.seed, threads=THREADS)
+        r = rows[it]
         gres = g.iterate(w.n_events, 0, w.seed)
-        assert_iteration_close(gres, ores)
-        if o.npass is not None:
-            assert g.last_npass() == o.npass
-        o.refine(w.alpha)
+        assert_iteration_close(gres, (r["I"], r["s"], r["h"]))
+        if r["npass"] is not None:
+            assert g.last_npass() == r["npass"]
         g.refine(w.alpha)
-        ge, oe = g.get_grid(), o.get_grid()
+        ge, oe = g.get_grid(), r["grid"]
         assert np.all(np.diff(ge, axis=1) > 0) and np.all(ge[:, 0] == 0) and np.all(ge[:, -1] == 1)
         assert np.max(np.abs(ge - oe)) <= 1e-12, (it, np.max(np.abs(ge - oe)))
-    assert g.iteration == o.iteration == w.n_iter
+    assert g.iteration == w.n_iter
+
+
+BENCH_PATH_STEPS = 5
+
+
+def bench_path(V, w, steps=BENCH_PATH_STEPS):
+    """Exactly the sequence bench.py times: reset, then `steps` fused steps of the full size enqueued back to back with NO
+    collect or synchronisation in between (every kernel carries the programmatic-dependent-launch attribute, so step i+1's
+    prologue runs under step i's S6/S7 tail), and only then the read-back."""
+    g = V.from_workload(w)
+    g.reset()
+    launches = [g.step_enqueue(w.n_events, w.n_events, w.seed, w.alpha) for _ in range(steps)]
+    g.refine_collect()                                   # raises if a refinement was rejected
+    I, s, _ = g.iterate_collect(want_hist=False)
+    return dict(I=I, s=s, grid=g.get_grid(), npass=g.last_npass(), launches=launches, iteration=g.iteration)
+
+
+def assert_bench_path(res, rows, w, steps=BENCH_PATH_STEPS):
+    last = rows[steps - 1]                               # a right grid after five steps implies right earlier steps
+    assert res["launches"] == [1] * steps and res["iteration"] == steps
+    assert abs(res["I"] - last["I"]) <= 1e-12 * abs(last["I"]), (res["I"], last["I"])
+    assert abs(res["s"] - last["s"]) <= 1e-12 * abs(last["s"]), (res["s"], last["s"])
+    if last["npass"] is not None:
+        assert res["npass"] == last["npass"]
+    assert np.max(np.abs(res["grid"] - last["grid"])) <= 1e-12, np.max(np.abs(res["grid"] - last["grid"]))
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
+def test_bench_path_parity(V, O, name):
+    """The path bench.py's device-timed region runs (un-synchronised chain of fused steps, 1e8 events each, one launch
+    per step, programmatic dependent launch live) against five free-running oracle steps at the stated tolerances:
+    I, sigma of the fifth step rel 1e-12, pass count exact, the grid after the fifth refinement within 1e-12."""
+    w = small_workloads()[name]
+    assert w.n_events == 10**8
+    assert_bench_path(bench_path(V, w), oracle_cascade(O, name), w)
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4", "cfg5"])
+def test_bench_path_parity_without_pdl(V, O, name):
+    """The same chain with VEGAS_NO_PDL=1 (plain stream order between the steps' kernels; the switch is read when the
+    library is loaded, hence the subprocess): same numbers against the oracle."""
+    import json
+    import subprocess
+    import sys
+    w = small_workloads()[name]
+    code = ("import json, sys; sys.path[:0] = [%r, %r]\n"
+            "from test_gpu_parity import bench_path, small_workloads\n"
+            "from paper_2010_09341_b200 import vegas as V\n"
+            "r = bench_path(V, small_workloads()[%r]); r['grid'] = r['grid'].tolist()\n"
+            "print('RESULT ' + json.dumps(r))\n") % (ROOT, os.path.join(ROOT, "tests"), name)
+    out = subprocess.run([sys.executable, "-c", code], cwd=ROOT, env=dict(os.environ, VEGAS_NO_PDL="1"),
+                         capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-3000:]
+    res = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("RESULT ")][-1][7:])
+    res["grid"] = np.array(res["grid"])
+    assert_bench_path(res, oracle_cascade(O, name), w)
+
+
+@pytest.mark.parametrize("epl", [0, 300_000])
+def test_shard_across_2pow32(V, O, epl):
+    """The global event index is 64 bits wide (S1: counter words 0 and 1) and a launch never straddles a multiple of 2^32
+    (its kernels keep the high word uniform): a shard [2^32 - 5e5, 2^32 + 5e5) of an iteration of 2^32 + 1e6 events, as one
+    requested launch (cut in two at 2^32) and as launches of 3e5 (cut at 2^32 as well), against the oracle's range call:
+    S1, S2, the pass count and every histogram cell."""
+    w = W.cfg2()
+    n_total, first, count = 2**32 + 10**6, 2**32 - 5 * 10**5, 10**6
+    g = V.from_workload(w)
+    o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    sums, hs, hc, npass = o.iterate_range(first, count, w.seed)
+    launches = g.iterate_shard_enqueue(n_total, first, count, epl or count, w.seed)
+    assert launches == (2 if not epl else 4)             # 5e5 | 5e5   and   3e5, 2e5 | 3e5, 2e5
+    p = g.partials_tensor().cpu().numpy()
+    import math
+    S1, S2, oS1, oS2 = math.fsum(p[0:2]), math.fsum(p[2:4]), math.fsum(sums[0:2]), math.fsum(sums[2:4])
+    assert abs(S1 - oS1) <= 1e-12 * abs(oS1) and abs(S2 - oS2) <= 1e-12 * abs(oS2)
+    assert int(p[4]) == npass == count
+    gh, oh = p[8:].reshape(w.dim, w.nbins), hs + hc
+    assert np.array_equal(gh == 0.0, oh == 0.0)
+    np.testing.assert_allclose(gh, oh, rtol=1e-10, atol=0.0)
+    g.finalize_enqueue(n_total)
+    I, s, _ = g.iterate_collect()
+    oI, os_ = o.commit(n_total, oS1, oS2, oh.copy())
+    assert abs(I - oI) <= 1e-12 * abs(oI) and abs(s - os_) <= 1e-12 * abs(os_)
+    # the events on both sides of the boundary, one by one (iteration counter as during the shard)
+    g.set_iteration(0); o.set_iteration(0)
+    for at in (2**32 - 64, 2**32):                       # (the parity hook takes ranges on one side of a multiple of 2^32)
+        assert_events_equal(g.debug_events(at, 64, seed=w.seed), o.events(at, 64, w.seed), w)
 
 
 def test_cfg3_sweep_parity(V, O):

@@ -19,6 +19,8 @@ def exact_combine(I, s):
     return float(mean), math.sqrt(float(1 / sw)), float(chi2 / (len(I) - 1)) if len(I) > 1 else 0.0
 
 
+LATE_RTOL = 1e-12          # iterations 6..20 of the 20-iteration graph test (see there)
+
 CASES = [([1.0, 2.0, 4.0], [1.0, 2.0, 4.0]),            # hand case: mean 4/3, error sqrt(16/21), chi2/dof 1/3
          ([0.5, 0.25, 0.75, 0.625], [0.125, 0.5, 0.25, 1.0]),
          ([3.0], [0.5]),
@@ -75,9 +77,9 @@ def test_run_integration_parity(name, n, epl, warm):
     o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
     gm, ge, gc, info = g.run_integration(4, n, epl, w.seed, w.alpha, n_warmup=warm)
     om, oe, oc, oI, os_ = o.run_integration(4, n, w.seed, w.alpha, n_warmup=warm, threads=8)
-    np.testing.assert_allclose(info["integral"], oI, rtol=1e-11)
-    np.testing.assert_allclose(info["error"], os_, rtol=1e-11)
-    assert gm == pytest.approx(om, rel=1e-11) and ge == pytest.approx(oe, rel=1e-11)
+    np.testing.assert_allclose(info["integral"], oI, rtol=1e-12)     # north_star's tolerance: at most 6 iterations here
+    np.testing.assert_allclose(info["error"], os_, rtol=1e-12)
+    assert gm == pytest.approx(om, rel=1e-12) and ge == pytest.approx(oe, rel=1e-12)
     assert gc == pytest.approx(oc, rel=1e-6, abs=1e-9)
     assert g.iteration == o.iteration == 4 + warm and np.all(info["kernel_ms"] > 0)
     assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
@@ -111,11 +113,20 @@ def test_run_integration_parity_across_a_multi_step_graph():
     o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
     gm, ge, gc, info = g.run_integration(18, w.n_events, 0, w.seed, w.alpha, n_warmup=2)
     om, oe, oc, oI, os_ = o.run_integration(18, w.n_events, w.seed, w.alpha, n_warmup=2, threads=8)
-    np.testing.assert_allclose(info["integral"], oI, rtol=1e-10)
-    np.testing.assert_allclose(info["error"], os_, rtol=1e-10)
-    assert gm == pytest.approx(om, rel=1e-10) and ge == pytest.approx(oe, rel=1e-10)
+    dI = np.abs(info["integral"] - oI) / np.abs(oI)
+    ds = np.abs(info["error"] - os_) / np.abs(os_)
+    dE = np.max(np.abs(g.get_grid() - o.get_grid()))
+    print("16-step graph, cfg1 x20: max rel dev I %.2e sigma %.2e over the first 5 | I %.2e sigma %.2e over all 20 | edges %.2e"
+          % (dI[:5].max(), ds[:5].max(), dI.max(), ds.max(), dE))
+    # the five iterations configs[0] states, at north_star's tolerance ...
+    assert dI[:5].max() <= 1e-12 and ds[:5].max() <= 1e-12
+    # ... and the fifteen beyond them, where the adaptive feedback amplifies last-bit differences of the histogram sums
+    # from refinement to refinement: measured I 7e-16, sigma 6e-14, edges 4e-14 by iteration 20, so
+    # the same tolerance still holds with a factor 16 to spare
+    assert dI.max() <= LATE_RTOL and ds.max() <= LATE_RTOL
+    assert gm == pytest.approx(om, rel=LATE_RTOL) and ge == pytest.approx(oe, rel=LATE_RTOL)
     assert g.iteration == o.iteration == 20 and np.all(info["kernel_ms"] > 0)
-    assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-10
+    assert dE <= LATE_RTOL
 
 
 @pytest.mark.gpu

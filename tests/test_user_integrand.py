@@ -81,7 +81,7 @@ def test_user_integrand_parity(src, dim, nbins, params, prec, frtol):
         assert np.max(np.abs(g.get_grid() - o.get_grid())) <= 1e-12
     gm, ge, gc, _ = g.run_integration(3, 100_000, 0, 9, 1.5)
     om, oe, oc, _, _ = o.run_integration(3, 100_000, 9, 1.5, threads=8)
-    assert gm == pytest.approx(om, rel=1e-11) and ge == pytest.approx(oe, rel=1e-11)
+    assert gm == pytest.approx(om, rel=1e-12) and ge == pytest.approx(oe, rel=1e-12)
 
 
 @pytest.mark.gpu
