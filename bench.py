@@ -40,23 +40,38 @@ UNIT = "events/s"
 ALGO_FLOPS = {"cfg1": 67.0, "cfg2": 154.0, "cfg2_u32": 154.0, "cfg4": 232.0, "cfg5": (130.0, 14.0)}
 # FP pipe lanes per SM (B200): 64 fp64, 128 fp32.  Peak = SMs * lanes * 2 FLOP * max SM clock.
 FP_LANES = {"f64": 64, "f32": 128}
-# What one launch of the committed iterate kernel executed per event and moved through DRAM, from the round-2 ncu
-# captures (profiles/r02_kernel_counts.md names the commands; written by `python -m paper_2010_09341_b200.ncu_counts`).
+# What one launch of the committed iterate kernel executed per event and moved through DRAM, from the round-3 ncu
+# captures (profiles/r03_kernel_counts.md names the commands; written by `python -m paper_2010_09341_b200.ncu_counts`).
 # The algorithmic HBM traffic is ~0: one table read and one d*N flush per CTA.
-KERNEL_COUNTS_CSV = os.path.join(ROOT, "profiles", "r02_kernel_counts.csv")
+KERNEL_COUNTS_CSV = os.path.join(ROOT, "profiles", "r03_kernel_counts.csv")
 
 
-def kernel_counts(workload):
-    """Row of profiles/r02_kernel_counts.csv for this workload (dict of floats), or None."""
+def kernel_counts(workload, w=None, shape=None):
+    """(row, note): the row of profiles/r03_kernel_counts.csv for this workload (dict of floats) -- or (None, why) when
+    there is none, when the kernel sources changed since the capture (the row's src_sha is not this tree's), or when the
+    instance the row was captured from, iterate_kernel<F, D, NB, RS, TREP, HB, MAXT, MINB>, is not the shape running
+    now (dim, bins, 2^RS histogram replicas, threads per CTA): stale counts must not pass for co-bounds."""
     import csv
+    import re
+    from paper_2010_09341_b200 import build as B
     try:
         with open(KERNEL_COUNTS_CSV) as fh:
-            for row in csv.DictReader(fh):
-                if row["workload"] == workload:
-                    return {k: (float(v) if k not in ("workload", "kernel") else v) for k, v in row.items()}
+            rows = [r for r in csv.DictReader(fh) if r["workload"] == workload]
     except OSError:
-        pass
-    return None
+        return None, "no %s" % os.path.relpath(KERNEL_COUNTS_CSV, ROOT)
+    if not rows:
+        return None, "no row for %s in %s" % (workload, os.path.relpath(KERNEL_COUNTS_CSV, ROOT))
+    row = rows[0]
+    text = ("workload", "kernel", "src_sha")
+    kc = {k: (v if k in text else float(v)) for k, v in row.items()}
+    if kc.get("src_sha") != B.kernel_source_sha():
+        return None, "the kernel sources changed since the capture (csv %s, tree %s): recapture" % (kc.get("src_sha"), B.kernel_source_sha())
+    m = re.search(r"<\s*\w+\s*,\s*(\d+),\s*(\d+),\s*(-?\d+),\s*(\d+),\s*(\d+),\s*(\d+),\s*(\d+)\s*>", kc["kernel"])
+    if m and w is not None and shape is not None:
+        D, NB, RS, _, _, MAXT, _ = (int(v) for v in m.groups())
+        if (D, NB) != (w.dim, w.nbins) or (RS >= 0 and (1 << RS) != shape["hist_replicas"]) or MAXT < shape["threads_per_cta"]:
+            return None, "captured instance %s is not the running shape %s" % (kc["kernel"], shape)
+    return kc, None
 
 
 def parse_args():
@@ -72,6 +87,7 @@ def parse_args():
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--replicas", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="skip the other_configs block (cfg1, cfg3, cfg4, cfg5)")
     ap.add_argument("--cpu-sample", type=int, default=10**8, help="events of the cpu_baseline oracle step")
     ap.add_argument("--ref-sample", type=int, default=10**7, help="events per step of --impl reference")
     ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
@@ -224,6 +240,79 @@ def nccl_lines(path, limit=12):
     return keep[:limit]
 
 
+def other_configs(V, torch, info, clock_hz, steps=5):
+    """The BASELINE.json configurations besides the headline one, so that the driver's record carries them too: device
+    time (CUDA events on the stream the kernels are launched on, which is torch's current stream) of `steps` whole
+    steps after 2 untimed ones.  cfg1: fused steps replayed by vegas_run_integration's CUDA graphs (the latency-bound
+    case: microseconds per step); cfg3: one iteration + refinement per events_per_launch of the batch-size study;
+    cfg4, cfg5: fused steps as in the headline measurement.  roofline_frac = algorithmic FLOPs (ALGO_FLOPS) per second
+    over SMs x lanes x 2 x max SM clock of the dtype's pipe."""
+    def frac(w, name, events_per_s, pass_fraction=1.0):
+        fpe = ALGO_FLOPS[name]
+        if isinstance(fpe, tuple):
+            fpe = fpe[0] * pass_fraction + fpe[1] * (1.0 - pass_fraction)
+        peak = info["sm_count"] * FP_LANES[dtype_of(w)] * 2 * clock_hz
+        return fpe * events_per_s / peak
+
+    def timed(fn, n_steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(n_steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / n_steps
+
+    out = {}
+    # cfg1: 1e5 events per step; 160 graph-replayed steps after a 16-step warm-up run
+    w = W.cfg1()
+    g = V.from_workload(w)
+    g.run_integration(16, w.n_events, 0, w.seed, w.alpha)
+    g.run_integration(160, w.n_events, 0, w.seed, w.alpha)
+    ms = g.last_sums()[2]                                 # the run's average device time per step
+    out["cfg1"] = {"us_per_step": ms * 1e3, "events_per_s": w.n_events / (ms * 1e-3), "steps": 160,
+                   "roofline_frac": frac(w, "cfg1", w.n_events / (ms * 1e-3)), "dtype": dtype_of(w),
+                   "path": "vegas_run_integration (CUDA graphs of 16 fused steps)"}
+    g.close()
+    # cfg3: the batch-size study
+    w = W.cfg3()
+    g = V.from_workload(w)
+    rows = []
+    for epl in w.batch_sizes:
+        g.reset()
+
+        def step():
+            g.iterate_enqueue(w.n_events, epl, w.seed)
+            g.refine_enqueue(w.alpha)
+        for _ in range(2):
+            step()
+        ms = timed(step, steps)
+        g.refine_collect()
+        rows.append({"events_per_launch": epl, "ms_per_iter": ms, "events_per_s": w.n_events / (ms * 1e-3),
+                     "roofline_frac": frac(w, "cfg2", w.n_events / (ms * 1e-3))})
+    out["cfg3"] = {"rows": rows, "dtype": dtype_of(w), "steps": steps, "path": "vegas_iterate_enqueue + vegas_refine_enqueue"}
+    g.close()
+    for name in ("cfg4", "cfg5"):
+        w = W.ALL[name]()
+        g = V.from_workload(w)
+        g.reset()
+
+        def step():
+            g.step_enqueue(w.n_events, w.n_events, w.seed, w.alpha)
+        for _ in range(2):
+            step()
+        ms = timed(step, steps)
+        g.refine_collect()
+        g.iterate_collect(want_hist=False)
+        pf = g.last_npass() / float(w.n_events)
+        out[name] = {"ms_per_iter": ms, "events_per_s": w.n_events / (ms * 1e-3), "steps": steps, "dtype": dtype_of(w),
+                     "roofline_frac": frac(w, name, w.n_events / (ms * 1e-3), pf), "pass_fraction": pf,
+                     "path": "vegas_step_enqueue (fused step)"}
+        g.close()
+    return out
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -336,29 +425,37 @@ def run_b200(args):
         achieved = flops / kern_s / 1e12
         fp_rate = pipes["dfma" if dt == "f64" else "ffma"]
         peak_measured = 2.0 * fp_rate / 1e12
-        # ---- the four co-bounds (SURVEY 8.d "Report all four"): fraction of each SM resource's measured rate that this
-        # kernel's own instruction stream takes at the measured events/s; per-event counts from the ncu capture of the
-        # committed kernel (profiles/r02_kernel_counts.csv), rates from vegas_pipe_rate in this process
-        kc = kernel_counts(args.workload)
+        # ---- the co-bounds (SURVEY 8.d "Report all four"): fraction of each SM resource's peak that this kernel's own
+        # instruction stream takes at the measured events/s; per-event counts from the ncu capture of the committed
+        # kernel (profiles/r03_kernel_counts.csv), pipe rates from vegas_pipe_rate in this process.  The shared-memory
+        # data pipe serves one wavefront per clock per SM; the issue stage one warp instruction per SM sub-partition
+        # per clock.  `evidence` holds comparison figures that are NOT hardware ceilings.
+        kc, kc_note = kernel_counts(args.workload, w, shape)
         ev_per_s = count / kern_s
-        bounds, bound_detail = None, None
+        bounds, bound_detail, evidence = None, {"note": kc_note}, None
         if kc:
-            issue_rate = info["sm_count"] * 4 * 32 * clock_hz          # one warp instruction per SM sub-partition per cycle
+            issue_rate = info["sm_count"] * 4 * 32 * clock_hz
             bounds = {
                 "fp_pipe": ev_per_s * kc["fp64" if dt == "f64" else "fp32"] / fp_rate,
                 "int_wide": ev_per_s * kc["imad_wide"] / pipes["imad_wide"],
-                "shared_atomic": ev_per_s * w.dim / pipes["shared_f64_add"],
+                "shared_pipe": ev_per_s * kc["smem_wavefronts"] / (info["sm_count"] * clock_hz),
                 "issue": ev_per_s * kc["inst"] / issue_rate,
-                # the same instruction count against the issue rate a dependency-free synthetic stream of the event loop's
-                # instruction ratio reaches (vegas_pipe_rate MIX_EVENT_LOOP): ~1 means the kernel issues as fast as its mix can
-                "issue_vs_synthetic_mix": ev_per_s * kc["inst"] / pipes["mix_event_loop"],
             }
-            bound_detail = {"per_event": {k: kc[k] for k in ("inst", "fp64", "fp32", "imad_wide", "imad", "lop3", "lds", "atoms")},
-                            "hist_updates_per_event": w.dim,
-                            "source": "profiles/r02_kernel_counts.csv (ncu capture of %s)" % kc["kernel"],
-                            "meaning": "events/s x per-event count / measured rate of that resource (1.0 = saturated); "
-                                       "shared_atomic counts the d histogram updates against the measured LDS+DADD+ATOMS.CAS update rate; "
-                                       "issue_vs_synthetic_mix is not a hardware ceiling but the rate of a stream with the loop's mix and no dependencies"}
+            evidence = {
+                # histogram updates that reach the accumulators (events that pass the cuts x d) against the rate of a
+                # latency-chained microbenchmark of the same LDS + DADD + ATOMS.CAS update (vegas_pipe_rate SHARED_F64_ADD)
+                "hist_updates_vs_cas_microbenchmark": ev_per_s * pass_fraction * w.dim / pipes["shared_f64_add"],
+                # the kernel's instruction rate against that of a dependency-free synthetic stream of the event loop's
+                # instruction ratio (vegas_pipe_rate MIX_EVENT_LOOP): a comparison stream, not a ceiling
+                "instr_rate_vs_synthetic_mix": ev_per_s * kc["inst"] / pipes["mix_event_loop"],
+            }
+            bound_detail = {"per_event": {k: kc[k] for k in ("inst", "fp64", "fp32", "imad_wide", "imad", "lop3", "lds", "atoms", "smem_wavefronts")},
+                            "hist_updates_per_event": w.dim * pass_fraction,
+                            "source": "profiles/r03_kernel_counts.csv (ncu capture of %s, kernel sources %s)" % (kc["kernel"], kc["src_sha"]),
+                            "meaning": "events/s x per-event count / peak rate of that resource (1.0 = saturated): fp_pipe and "
+                                       "int_wide against the measured DFMA|FFMA and IMAD.WIDE rates, shared_pipe = shared-memory "
+                                       "wavefronts against 1 per clock per SM, issue = warp instructions against 1 per clock per "
+                                       "SM sub-partition"}
         at_full = (n == w.n_events and world == 1 and epl == n)
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -372,7 +469,7 @@ def run_b200(args):
             "gpu_launches": launches,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": kc["dram_bytes"] if (kc and at_full) else None,
-                         "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture in profiles/r02_kernel_counts.csv",
+                         "traffic_unit": "bytes per launch: dram__bytes_read.sum + dram__bytes_write.sum of the ncu --set full capture in profiles/r03_kernel_counts.csv",
                          "kernel": "iterate_kernel", "kernel_ms": kern_s * 1e3,
                          "flops_per_event": fpe,
                          "peak_source": "SMs x %d %s lanes x 2 x max SM clock (B200 unit counts; DESIGN.md section 7)" % (FP_LANES[dt], dt),
@@ -380,10 +477,13 @@ def run_b200(args):
                          "peak_measured_source": "2 x vegas_pipe_rate(%s) in this process before the timed region" % ("DFMA" if dt == "f64" else "FFMA"),
                          "pipe_rates_thread_instr_per_s": pipes,
                          "bounds": bounds,
-                         "co_bound": max((k for k in bounds if k != "issue_vs_synthetic_mix"), key=bounds.get) if bounds else None,
+                         "co_bound": max(bounds, key=bounds.get) if bounds else None,
+                         "evidence": evidence,
                          "bounds_detail": bound_detail},
             "result": {"integral": I, "error": s, "pass_fraction": pass_fraction},
         }
+        if world == 1 and args.workload == "cfg2" and at_full and not args.no_other_configs:
+            out["other_configs"] = other_configs(V, torch, info, clock_hz)
         if world > 1:
             out["config"]["parallelism"] = ("events sharded over %d ranks ([g n/N, (g+1) n/N), last rank takes the remainder); one "
                                             "all-reduce of %d doubles per iteration (%s); identical refine on every rank"

@@ -32,6 +32,18 @@ NVCC_FLAGS = [
 ]
 
 
+def kernel_source_sha() -> str:
+    """First 16 hex digits of sha256 over the two headers that hold the device code of the iterate kernel.  Stored
+    with the per-event counts an ncu capture yields (ncu_counts.py) so that bench.py can tell whether those counts
+    still describe the kernels it is running."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in ("vegas_device.cuh", "vegas_kernels.cuh"):
+        with open(os.path.join(CSRC, name), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def nvcc_path() -> str:
     cand = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(cand):

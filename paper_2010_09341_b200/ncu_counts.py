@@ -6,15 +6,19 @@ Reads the report with `ncu -i <report> --page raw --csv` (whole-launch counters)
 count of every SASS instruction; needs --import-source at capture time and -lineinfo at compile time) and prints ONE
 csv row: what one launch executed, divided by the events it processed --
 
-    workload, kernel, n_events, kernel_us, dram_bytes, inst, fp64, fp32, imad_wide, imad, lop3, lds, atoms
+    workload, kernel, n_events, kernel_us, dram_bytes, inst, fp64, fp32, imad_wide, imad, lop3, lds, atoms,
+    smem_wavefronts, src_sha
 
 `inst` .. `atoms` are warp instructions x 32 / n_events = thread instructions per event (retries of lost histogram races
 included, predicated-off lanes counted: these are issue slots and pipe cycles, which is what bounds the kernel).
-bench.py reads the committed table (profiles/r02_kernel_counts.csv) for the co-bounds of its roofline block and for
-`roofline.traffic`; `--md` prints the opcode histogram as a markdown table instead (profiles/r02_sass_hist_*.md);
+`smem_wavefronts` = l1tex__data_pipe_lsu_wavefronts_mem_shared.sum / n_events: shared-memory data-pipe wavefronts per
+event (the pipe serves one per clock per SM); `src_sha` = build.kernel_source_sha() of the tree the report is parsed in
+(parse right after the capture, from the same tree).
+bench.py reads the committed table (profiles/r03_kernel_counts.csv) for the co-bounds of its roofline block and for
+`roofline.traffic`; `--md` prints the opcode histogram as a markdown table instead (profiles/r03_sass_hist_*.md);
 `--summary` prints the whole-launch counters the design discussion quotes (pipes, issue slots, shared-memory
 wavefronts and bank conflicts, DRAM bytes, stall reasons per issued instruction) as a markdown table
-(profiles/r02_ncu_full_*.md).  No GPU needed: ncu only parses the report.
+(profiles/r03_ncu_full_*.md).  No GPU needed: ncu only parses the report.
 """
 from __future__ import annotations
 
@@ -24,9 +28,11 @@ import re
 import subprocess
 import sys
 
+from . import build as _build
+
 FP64 = ("DADD", "DFMA", "DMUL", "DSETP")
 FP32 = ("FADD", "FFMA", "FMUL", "FSETP", "FSEL", "FMNMX", "FCHK", "MUFU")
-HEADER = "workload,kernel,n_events,kernel_us,dram_bytes,inst,fp64,fp32,imad_wide,imad,lop3,lds,atoms"
+HEADER = "workload,kernel,n_events,kernel_us,dram_bytes,inst,fp64,fp32,imad_wide,imad,lop3,lds,atoms,smem_wavefronts,src_sha"
 SUMMARY = """Kernel Name
 gpu__time_duration.sum
 launch__registers_per_thread
@@ -146,7 +152,8 @@ def main(argv):
     atoms = sum(v for k, v in cnt.items() if k.startswith("ATOMS"))
     row = [workload, '"%s"' % kernel, "%d" % n, "%.2f" % t, "%.0f" % dram, "%.2f" % (sum(cnt.values()) * per),
            "%.2f" % (family(cnt, FP64) * per), "%.2f" % (family(cnt, FP32) * per), "%.2f" % (wide * per), "%.2f" % (imad * per),
-           "%.2f" % (family(cnt, ("LOP3",)) * per), "%.2f" % (lds * per), "%.2f" % (atoms * per)]
+           "%.2f" % (family(cnt, ("LOP3",)) * per), "%.2f" % (lds * per), "%.2f" % (atoms * per),
+           "%.3f" % (float(raw.get("l1tex__data_pipe_lsu_wavefronts_mem_shared.sum", 0) or 0) / n), _build.kernel_source_sha()]
     print(",".join(row))
     return 0
 
