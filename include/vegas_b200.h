@@ -14,9 +14,9 @@
  *     error vegas_last_error() returns a static, thread-local, NUL-terminated description.
  *   - The caller owns every buffer it passes.  `params` is copied at create.  `dev_workspace` (device
  *     memory, >= vegas_workspace_bytes(), 256-byte aligned) and `cuda_stream` (a cudaStream_t cast to
- *     void*, NULL = the legacy default stream) are borrowed and must outlive the context; the library
+ *     void*, NULL = the legacy default stream) are borrowed and must outlive the context; the hot path
  *     allocates no device memory itself (every device buffer, the scratch of vegas_debug_events included, is a
- *     region of dev_workspace); it allocates a few hundred bytes of pinned host memory for results.
+ *     region of dev_workspace; the microbenchmark vegas_pipe_rate is the one exception, stated there); it allocates a few hundred bytes of pinned host memory for results.
  *   - A context is not thread-safe.  Calls that return results to host pointers are synchronous at
  *     return (they synchronise the stream); they enqueue asynchronously inside (no host sync between
  *     the launches of one iteration).
@@ -215,6 +215,11 @@ int vegas_iterate_shard_enqueue(vegas_ctx* ctx, uint64_t n_total, uint64_t first
                                 uint64_t events_per_launch, uint64_t seed, int* n_kernel_launches);
 int vegas_partials(const vegas_ctx* ctx, void** dev_partials, size_t* n_doubles);
 int vegas_finalize_enqueue(vegas_ctx* ctx, uint64_t n_total);
+/* vegas_finalize_enqueue + vegas_refine_enqueue(alpha) as ONE kernel (S6 by one thread beside the first steps of S7): the
+ * tail of a sharded step after the all-reduce.  Same numbers as the two calls; afterwards vegas_iterate_collect (without
+ * hist: it was consumed), vegas_last_sums, vegas_last_npass and vegas_refine_collect work as after them.
+ * Errors: those of the two calls. */
+int vegas_finalize_step_enqueue(vegas_ctx* ctx, uint64_t n_total, double alpha);
 
 /* Test hook: load H (dim*nbins doubles >= 0, row-major [k][i], host) as if a vegas_iterate had produced it, so that
  * hand-made histograms reach the refinement kernel (the independent pins of S7).  Synchronises.
@@ -302,7 +307,9 @@ int vegas_plan_launches(uint64_t n_events, uint64_t events_per_launch, int threa
  * one SM pipe the hot path is bound by -- the denominators of the "alu" roofline bench.py reports
  * (BASELINE.json north_star: "fraction of the FP pipe roofline").  Each call runs a
  * few milliseconds of 8 independent dependency chains per thread at full occupancy on `cuda_stream`
- * (NULL = default stream) and synchronises.  No context needed.
+ * (NULL = default stream) and synchronises.  No context needed -- and so no workspace: this benchmark call is the one
+ * place where the library allocates device memory itself (cudaMalloc / cudaFree of 8 KB per SM, 2.4 MB on a B200, for the
+ * chains' results); it is not part of the hot path.
  *   VEGAS_PIPE_DFMA            fp64 fused multiply-add   (peak FLOP/s = 2 x rate)
  *   VEGAS_PIPE_FFMA            fp32 fused multiply-add
  *   VEGAS_PIPE_IMAD_WIDE       32x32->64 integer multiply (two per Philox round)

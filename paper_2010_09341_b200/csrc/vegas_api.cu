@@ -1083,14 +1083,12 @@ int vegas_set_histogram(vegas_ctx* c, const double* hist)
     return VEGAS_OK;
 }
 
-int vegas_refine_enqueue(vegas_ctx* c, double alpha)
+// Launch geometry of the refinement CTA (refine_kernel, finalize_refine_kernel): all dimensions in one CTA, as many at a
+// time as fit in shared memory (at most one per warp); the steps that are independent per bin use ceil((N + 1) / 32)
+// warps per dimension when the CTA has them.
+static int refine_geometry(const vegas_ctx* c, int* cta_warps_out, size_t* smem_out, size_t* max_smem_out)
 {
-    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
-    if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
-    if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
     const int N = c->nbins;
-    // all dimensions in one CTA, as many at a time as fit in shared memory (at most one per warp); the steps that are
-    // independent per bin use ceil((N + 1) / 32) warps per dimension when the CTA has them
     const size_t per_dim = 4 * (static_cast<size_t>(N) + 1) * sizeof(double);
     const int warps = c->dim < 32 ? c->dim : 32;
     int cta_warps = warps * ((N + 1 + 31) / 32);
@@ -1099,6 +1097,59 @@ int vegas_refine_enqueue(vegas_ctx* c, double alpha)
     size_t smem = per_dim * static_cast<size_t>(warps);
     if (smem > max_smem) smem = (max_smem / per_dim) * per_dim;
     if (smem < per_dim) return fail(VEGAS_EINVAL, "nbins %d: one dimension's refinement does not fit in shared memory", N);
+    *cta_warps_out = cta_warps; *smem_out = smem; *max_smem_out = max_smem;
+    return VEGAS_OK;
+}
+
+namespace {
+// S6 and S7 in one launch: the sharded step after the all-reduce (vegas_finalize_step_enqueue).  S6 is one thread's
+// work on the summed partials header; it runs in the CTA's last warp, which has the fewest bins in S7's first steps.
+__global__ void finalize_refine_kernel(const double* partials, unsigned long long n_events, double* result, double* edges,
+                                       double* hist, int N, double alpha, double* new_edges, int d, void* table,
+                                       int precision, int* status, int smem_bytes)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if (threadIdx.x == blockDim.x - 1) estimate_s6(partials, n_events, result);
+    refine_all(edges, hist, N, alpha, new_edges, d, table, precision, status, smem_raw, static_cast<size_t>(smem_bytes), false);
+}
+}  // namespace
+
+int vegas_finalize_step_enqueue(vegas_ctx* c, uint64_t n_total, double alpha)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (n_total < 2) return fail(VEGAS_EINVAL, "n_events must be >= 2");
+    if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
+    if (!c->shard_pending) return fail(VEGAS_ESTATE, "vegas_finalize_step_enqueue follows vegas_iterate_shard_enqueue");
+    int cta_warps = 0;
+    size_t smem = 0, max_smem = 0;
+    const int rc = refine_geometry(c, &cta_warps, &smem, &max_smem);
+    if (rc != VEGAS_OK) return rc;
+    if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(finalize_refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(max_smem)));
+    finalize_refine_kernel<<<1, 32 * cta_warps, smem, c->stream>>>(
+        reinterpret_cast<const double*>(c->ws + c->L.part), n_total, reinterpret_cast<double*>(c->ws + c->L.result),
+        reinterpret_cast<double*>(c->ws + c->L.edges), reinterpret_cast<double*>(c->ws + c->L.hist), c->nbins, alpha,
+        reinterpret_cast<double*>(c->ws + c->L.new_edges), c->dim, c->ws + c->L.table, c->precision == VEGAS_FP32_EVAL ? 1 : 0,
+        reinterpret_cast<int*>(c->ws + c->L.status), static_cast<int>(smem));
+    CUDA_TRY(cudaGetLastError());
+    c->shard_pending = false;
+    c->have_sums = true;
+    c->last_n = n_total;
+    c->have_hist = false;                                // consumed by the refinement (vegas_refine_collect hands it back
+    c->hist_consumed = true;                             // if the refinement is rejected)
+    c->refine_pending += 1;
+    return VEGAS_OK;
+}
+
+int vegas_refine_enqueue(vegas_ctx* c, double alpha)
+{
+    if (!c) return fail(VEGAS_EINVAL, "ctx is NULL");
+    if (!(alpha >= 0.0)) return fail(VEGAS_EINVAL, "alpha must be >= 0");
+    if (!c->have_hist) return fail(VEGAS_ESTATE, "vegas_refine needs the histogram of a vegas_iterate");
+    const int N = c->nbins;
+    int cta_warps = 0;
+    size_t smem = 0, max_smem = 0;
+    const int rc = refine_geometry(c, &cta_warps, &smem, &max_smem);
+    if (rc != VEGAS_OK) return rc;
     if (smem > 48 * 1024) CUDA_TRY(cudaFuncSetAttribute(refine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(max_smem)));
     double* edges = reinterpret_cast<double*>(c->ws + c->L.edges);
     double* new_edges = reinterpret_cast<double*>(c->ws + c->L.new_edges);

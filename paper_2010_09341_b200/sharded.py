@@ -28,10 +28,12 @@ def shard_range(n_events: int, rank: int, world: int):
 
 
 def iterate_sharded_enqueue(ctx, n_events: int, events_per_launch: int = 0, seed: int = 0, group=None,
-                            rank: int | None = None, world: int | None = None):
+                            rank: int | None = None, world: int | None = None, refine_alpha: float | None = None):
     """One sharded iteration: this rank's shard, ONE all-reduce of the partials, S6.  Returns the number of kernels this
     rank launched for its shard.  Without an initialised process group (or world == 1) the shard is the whole range and
-    no collective runs.  Results are read afterwards with ctx.iterate_collect() like after a plain iteration."""
+    no collective runs.  Results are read afterwards with ctx.iterate_collect() like after a plain iteration.
+    With refine_alpha the identical refinement of every rank is part of the call -- S6 and S7 run as one kernel after
+    the all-reduce (ctx.finalize_step_enqueue) -- and its outcome is read with ctx.refine_collect()."""
     import torch.distributed as dist
     have_pg = dist.is_available() and dist.is_initialized()
     if world is None:
@@ -54,7 +56,10 @@ def iterate_sharded_enqueue(ctx, n_events: int, events_per_launch: int = 0, seed
                 dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
         else:
             dist.all_reduce(part, op=dist.ReduceOp.SUM, group=group)
-    ctx.finalize_enqueue(int(n_events))
+    if refine_alpha is None:
+        ctx.finalize_enqueue(int(n_events))
+    else:
+        ctx.finalize_step_enqueue(int(n_events), float(refine_alpha))
     return launches
 
 

@@ -45,6 +45,7 @@ SIGNATURES = {
     "vegas_iterate_shard_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, C.c_uint64, _ip]),
     "vegas_partials": (C.c_int, [_vp, C.POINTER(_vp), _szp]),
     "vegas_finalize_enqueue": (C.c_int, [_vp, C.c_uint64]),
+    "vegas_finalize_step_enqueue": (C.c_int, [_vp, C.c_uint64, C.c_double]),
     "vegas_set_histogram": (C.c_int, [_vp, _dp]),
     "vegas_set_launch_shape": (C.c_int, [_vp, C.c_int, C.c_int]),
     "vegas_set_hist_replicas": (C.c_int, [_vp, C.c_int]),
@@ -251,6 +252,10 @@ class Vegas:
 
     def finalize_enqueue(self, n_total):
         _chk(lib().vegas_finalize_enqueue(self._h, int(n_total)), "vegas_finalize_enqueue")
+
+    def finalize_step_enqueue(self, n_total, alpha):
+        """S6 from the summed partials and the refinement, one kernel (the tail of a sharded step)."""
+        _chk(lib().vegas_finalize_step_enqueue(self._h, int(n_total), float(alpha)), "vegas_finalize_step_enqueue")
 
     def set_histogram(self, hist):
         h = np.ascontiguousarray(hist, dtype=np.float64)

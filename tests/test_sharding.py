@@ -123,6 +123,63 @@ def test_sharded_iteration_two_ranks_one_gpu_non_default_stream(V):
 
 
 @pytest.mark.gpu
+@pytest.mark.parametrize("name,n", [("cfg2", 10**6 + 3), ("cfg4", 300_007)])
+def test_finalize_step_is_finalize_plus_refine(V, name, n):
+    """vegas_finalize_step_enqueue (S6 + S7 in one kernel after the all-reduce) against the oracle: two shards into two
+    contexts, partials summed on the device, then the fused tail; I, sigma rel 1e-12, grid within 1e-12, two iterations."""
+    from oracle import oracle as O
+    w = W.ALL[name]()
+    o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    ctxs = [V.from_workload(w) for _ in range(2)]
+    for it in range(2):
+        oI, os_, _ = o.iterate(n, w.seed, threads=THREADS)
+        o.refine(w.alpha)
+        for rank, c in enumerate(ctxs):
+            first, count = sharded.shard_range(n, rank, 2)
+            c.iterate_shard_enqueue(n, first, count, count, w.seed)
+        parts = [c.partials_tensor() for c in ctxs]
+        total = parts[0] + parts[1]
+        for p, c in zip(parts, ctxs):
+            p.copy_(total)
+            c.finalize_step_enqueue(n, w.alpha)
+            I, s, _ = c.iterate_collect(want_hist=False)
+            c.refine_collect()
+            assert abs(I - oI) <= 1e-12 * abs(oI) and abs(s - os_) <= 1e-12 * abs(os_)
+            assert np.max(np.abs(c.get_grid() - o.get_grid())) <= 1e-12
+            with pytest.raises(V.VegasError) as ei:
+                c.iterate_collect(want_hist=True)            # consumed by the refinement
+            assert ei.value.code == V.ESTATE
+        assert np.array_equal(ctxs[0].get_grid(), ctxs[1].get_grid())
+    with pytest.raises(V.VegasError) as ei:
+        ctxs[0].finalize_step_enqueue(n, w.alpha)            # no shard pending
+    assert ei.value.code == V.ESTATE
+
+
+@pytest.mark.gpu
+def test_bench_two_ranks_gloo_on_one_gpu_matches_the_oracle(V):
+    """bench.py's N > 1 path (sharded strong scaling: shard, one all-reduce, fused S6 + S7 on every rank) under
+    torch.distributed.run with two gloo ranks sharing the one GPU: its line says so and its result is the oracle's."""
+    import json
+    from oracle import oracle as O
+    n, steps, warm = 2_000_003, 2, 1
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), "bench.py", "--gpus", "2", "--dist-backend", "gloo", "--workload", "cfg2",
+           "--n-events", str(n), "--steps", str(steps), "--warmup", str(warm)]
+    r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, OMP_NUM_THREADS="1"), capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-3000:]
+    line = json.loads([ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == "strong" and "parallelism" in line["config"]
+    assert line["gpu_launches"] == 2 * steps
+    w = W.cfg2()
+    o = O.Oracle(w.dim, w.nbins, w.integrand_id, w.params, w.precision)
+    for _ in range(warm + steps):                            # the device-timed region's last step, from a reset grid
+        oI, os_, _ = o.iterate(n, w.seed, threads=THREADS)
+        o.refine(w.alpha)
+    assert abs(line["result"]["integral"] - oI) <= 1e-12 * abs(oI)
+    assert abs(line["result"]["error"] - os_) <= 1e-12 * abs(os_)
+
+
+@pytest.mark.gpu
 def test_shard_argument_errors(V):
     w = W.cfg1()
     g = V.from_workload(w)
